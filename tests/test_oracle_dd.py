@@ -1,0 +1,292 @@
+"""Pins for the oracle's domain-decomposition loops (Sec. 3, :129-182; DESIGN.md readings).
+
+The attempt trace is checked against what the paper fixes: 1 MCS = L^2 attempts (:106); four
+non-interacting domain sets that are visited in a shuffled permutation (:144); every thread cell
+receives exactly one attempt per collective step (:168); DB cells are the aligned cells displaced by
+one common random origin and wrap inside the domain (:172, R14); DT picks one quadrant per step (:170);
+dead-border hits are not carried out (:135).  Order independence, split invariance and the
+deposition/removal symmetry pin the loop nest against dropped or transposed indices.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import BLK_DB, BLK_DB_DELAYED, BLK_DT, DEV_CDB, DEV_DB, DEV_DT, DEV_DTR, Oracle, scheme
+
+
+def run_traced(L, seed, code, n_mcs, p=1.0, q=0.0, t0=0):
+    o = Oracle(L, seed)
+    if t0:
+        o.set_lattice(o.lattice.copy(), t=t0)
+    o.start_trace(n_mcs * L * L + 16)
+    o.sweep(n_mcs, p, q, code)
+    tr = o.stop_trace()
+    return o, tr
+
+
+def dims(code):
+    return 1 << ((code >> 16) & 31), 4 << ((code >> 8) & 15), 4 << ((code >> 12) & 15)
+
+
+@pytest.mark.parametrize("code", [scheme(DEV_DTR, BLK_DB, 5), scheme(DEV_DTR, BLK_DB, 5, 2, 1),
+                                  scheme(DEV_DT, BLK_DB_DELAYED, 5), scheme(DEV_DTR, BLK_DB, 4, 0, 0)])
+def test_dtr_db_trace_geometry(code):
+    L, seed = 128, 21
+    D, cx, cy = dims(code)
+    dev = code & 15
+    o, tr = run_traced(L, seed, code, 2, p=0.6, q=0.4 if (code >> 4) & 15 == BLK_DB_DELAYED else 0.0)
+    assert len(tr) == 2 * L * L                                        # :106
+    nt = L // (2 * D)
+    for t in (0, 1):
+        Ox, Oy, perm = oracle.mcs_control(seed, t, L, dev)
+        if dev == DEV_DT:
+            assert (Ox, Oy) == (0, 0)
+        rec = tr[tr["t"] == t]
+        # sets appear in the order of the permutation, each one complete before the next (:144)
+        set_seq = [k for k, _ in itertools.groupby(rec["set"].tolist())]
+        assert tuple(set_seq) == perm and sorted(perm) == [0, 1, 2, 3]
+        cover = np.zeros((L, L), dtype=np.int32)
+        for s in range(4):
+            rs = rec[rec["set"] == s]
+            assert len(rs) == L * L // 4
+            assert set(rs["dom"].tolist()) == set(range(nt * nt))
+            for dom in range(nt * nt):
+                rd = rs[rs["dom"] == dom]
+                assert len(rd) == D * D                                # one sweep of the domain (R12)
+                I, J = dom % nt, dom // nt
+                gx = (Ox + 2 * D * I + (s & 1) * D) % L
+                gy = (Oy + 2 * D * J + (s >> 1) * D) % L
+                lx = (rd["x"].astype(np.int64) - gx) % L
+                ly = (rd["y"].astype(np.int64) - gy) % L
+                assert (lx < D).all() and (ly < D).all()               # inside its own sub-tile
+                cover[gy:gy + 1, gx:gx + 1] += 0
+                yy = (gy + np.arange(D)) % L
+                xx = (gx + np.arange(D)) % L
+                cover[np.ix_(yy, xx)] += 1
+                ncx = D // cx
+                for k in range(cx * cy):
+                    rk = rd[rd["k"] == k]
+                    assert sorted(rk["cell"].tolist()) == list(range((D // cx) * (D // cy)))   # single hit (:168)
+                    a, b = rk["cell"] % ncx, rk["cell"] // ncx
+                    klx, kly = (rk["x"].astype(np.int64) - gx) % L, (rk["y"].astype(np.int64) - gy) % L
+                    # one common origin (ox,oy) per step explains every cell's site (:172, R13/R14)
+                    ok = [(ox, oy) for ox in range(cx) for oy in range(cy)
+                          if ((((klx - ox) % D) // cx) == a).all() and ((((kly - oy) % D) // cy) == b).all()]
+                    assert len(ok) >= 1
+                    ox, oy = ok[0]
+                    inx, iny = (klx - ox) % D - a * cx, (kly - oy) % D - b * cy
+                    cls = (inx == cx - 1).astype(int) + (iny == cy - 1).astype(int)
+                    if len(ok) == 1:
+                        assert (cls == rk["cls"]).all()                # +x column / +y row are the border (R15)
+        assert (cover == 1).all()                                      # the 4 sets tile the lattice exactly
+    o.close()
+
+
+def test_delayed_phases_are_ordered_bulk_edges_corners():
+    code = scheme(DEV_DTR, BLK_DB_DELAYED, 5)
+    o, tr = run_traced(64, 4, code, 1, p=0.5, q=0.5)
+    for (s, d, k), grp in itertools.groupby(tr, key=lambda r: (r["set"], r["dom"], r["k"])):
+        cls = [int(r["cls"]) for r in grp]
+        assert cls == sorted(cls)                                      # :174 "corners ... last"
+    o.close()
+
+
+@pytest.mark.parametrize("code", [scheme(DEV_DTR, BLK_DT, 5), scheme(DEV_DTR, BLK_DT, 5, 2, 1)])
+def test_dt_block_layer_trace(code):
+    L, seed = 64, 8
+    D, cx, cy = dims(code)
+    o, tr = run_traced(L, seed, code, 2)
+    assert len(tr) == 2 * L * L
+    quads = []
+    for t in (0, 1):
+        Ox, Oy, perm = oracle.mcs_control(seed, t, L, DEV_DTR)
+        rec = tr[tr["t"] == t]
+        nt = L // (2 * D)
+        for s in range(4):
+            for dom in range(nt * nt):
+                rd = rec[(rec["set"] == s) & (rec["dom"] == dom)]
+                gx = (Ox + 2 * D * (dom % nt) + (s & 1) * D) % L
+                gy = (Oy + 2 * D * (dom // nt) + (s >> 1) * D) % L
+                lx, ly = (rd["x"].astype(np.int64) - gx) % L, (rd["y"].astype(np.int64) - gy) % L
+                assert (lx < D).all() and (ly < D).all()
+                a, b = rd["cell"] % (D // cx), rd["cell"] // (D // cx)
+                assert ((lx // cx) == a).all() and ((ly // cy) == b).all()     # aligned cells, no wrap
+                qx, qy = (lx % cx) // (cx // 2), (ly % cy) // (cy // 2)
+                for k in range(cx * cy):
+                    m = rd["k"] == k
+                    assert m.sum() == (D // cx) * (D // cy)
+                    assert len(set(qx[m].tolist())) == 1 and len(set(qy[m].tolist())) == 1   # one quadrant per step (R17)
+                    quads.append(int(qx[m][0]) + 2 * int(qy[m][0]))
+    # drawn with replacement, all four occur, roughly uniformly (:170 "at random", not a permutation)
+    cnt = np.bincount(quads, minlength=4)
+    assert (cnt > 0.15 * len(quads)).all()
+    runs = sum(1 for i in range(0, len(quads) - 3, 4) if sorted(quads[i:i + 4]) == [0, 1, 2, 3])
+    assert runs < 0.5 * (len(quads) // 4)
+    o.close()
+
+
+@pytest.mark.parametrize("dev,w", [(DEV_DB, 5), (DEV_CDB, 1)])
+def test_dead_border_device_layer(dev, w):
+    L, seed, code = 128, 17, scheme(dev, BLK_DB, 5)
+    D = 32
+    o, tr = run_traced(L, seed, code, 3)
+    assert len(tr) == 3 * L * L
+    for t in range(3):
+        Ox, Oy, _ = oracle.mcs_control(seed, t, L, dev)
+        if dev == DEV_CDB:
+            assert Ox % 4 == 0 and Oy % 4 == 0                        # :166 coarse grid
+        rec = tr[tr["t"] == t]
+        lx = (rec["x"].astype(np.int64) - Ox) % D
+        ly = (rec["y"].astype(np.int64) - Oy) % D
+        border = (lx >= D - w) | (ly >= D - w)
+        assert ((rec["result"] == 2) == border).all()                 # border hits are not carried out (:135)
+        nt = L // D
+        dom = ((rec["y"].astype(np.int64) - Oy) % L) // D * nt + ((rec["x"].astype(np.int64) - Ox) % L) // D
+        assert (dom == rec["dom"]).all()
+        # Eq. (9), reading R9: the active fraction of a sweep
+        assert abs(border.mean() - (1 - ((D - w) / D) ** 2)) < 0.01
+    o.close()
+
+
+def test_origin_and_permutation_statistics():
+    L = 1024
+    ox, oy, perms = [], [], []
+    for t in range(4800):
+        a, b, p = oracle.mcs_control(99, t, L, DEV_DTR)
+        ox.append(a); oy.append(b); perms.append(p)
+    allp = list(itertools.permutations(range(4)))                     # lexicographic
+    cnt = np.array([perms.count(p) for p in allp])
+    assert (cnt > 120).all() and (cnt < 290).all()                    # 200 expected each
+    assert abs(np.mean(ox) - (L - 1) / 2) < 4 * L / np.sqrt(12 * 4800)
+    assert abs(np.mean(oy) - (L - 1) / 2) < 4 * L / np.sqrt(12 * 4800)
+    assert len(set(np.array(ox) % 4)) == 4                            # arbitrary site, not a coarse grid (:150)
+    # the permutation index is the lexicographic rank of G[2] % 24
+    for t in range(50):
+        G = oracle.philox4x32_10([0, 0, 2 << 30, t], [99, 0])
+        a, b, p = oracle.mcs_control(99, t, L, DEV_DTR)
+        assert p == allp[int(G[2]) % 24] and a == int(G[0]) % L and b == int(G[1]) % L
+
+
+def test_site_selection_is_uniform_under_dtrdb():
+    # every site has selection rate exactly 1/(cx*cy) per step (R14) -> Poisson-like counts, no site starved
+    L, n = 64, 60
+    o, tr = run_traced(L, 31, scheme(DEV_DTR, BLK_DB, 4), n)
+    cnt = np.zeros((L, L))
+    np.add.at(cnt, (tr["y"], tr["x"]), 1)
+    assert abs(cnt.mean() - n) < 1e-9
+    var = cnt.var()
+    assert 0.5 * n < var < 1.3 * n                                    # binomial-ish: var ~ n(1-1/64)
+    chi = ((cnt - n) ** 2 / n).sum() / (L * L)
+    assert 0.8 < chi < 1.2
+    o.close()
+
+
+ORDER_CASES = [
+    (scheme(DEV_DTR, BLK_DB, 5), 1.0, 0.0), (scheme(DEV_DTR, BLK_DB, 5), 0.0, 1.0),
+    (scheme(DEV_DTR, BLK_DB, 5), 0.9, 0.1), (scheme(DEV_DTR, BLK_DB_DELAYED, 5), 1.0, 0.0),
+    (scheme(DEV_DTR, BLK_DT, 5), 0.5, 0.5), (scheme(DEV_DT, BLK_DB, 5), 1.0, 0.0),
+    (scheme(DEV_DB, BLK_DB, 5), 0.9, 0.1), (scheme(DEV_CDB, BLK_DB, 5), 1.0, 0.0),
+    (scheme(DEV_DB, BLK_DT, 5), 1.0, 0.0), (scheme(DEV_DTR, BLK_DB, 5, 2, 2), 0.9, 0.1),
+    (scheme(DEV_DTR, BLK_DB, 5, 0, 0), 0.5, 0.5), (scheme(DEV_DTR, BLK_DB, 6, 3, 1), 1.0, 0.0),
+]
+
+
+@pytest.mark.parametrize("code,p,q", ORDER_CASES)
+def test_order_independence(code, p, q):
+    """Domains of one set, and cells within one phase, never touch common bits: any visiting order
+    gives the same lattice.  This is what lets a parallel machine reproduce the oracle bit for bit."""
+    L = 128
+    ref = Oracle(L, 77)
+    ref.sweep(6, p, q, code)
+    for sh in (1, 0xDEADBEEF, 12345678901):
+        o = Oracle(L, 77)
+        o.set_shuffle(sh)
+        o.sweep(6, p, q, code)
+        assert (o.lattice == ref.lattice).all() and o.net == ref.net and o.h00 == ref.h00
+        o.close()
+    ref.close()
+
+
+def test_sync_and_delayed_are_different_samples_of_the_same_process():
+    # R16: "completely equivalent" (:174) holds in distribution, not bit-wise
+    L = 128
+    a, b = Oracle(L, 5), Oracle(L, 5)
+    a.sweep(20, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 5))
+    b.sweep(20, 1.0, 0.0, scheme(DEV_DTR, BLK_DB_DELAYED, 5))
+    assert (a.lattice != b.lattice).any()
+    assert abs(a.net - b.net) < 0.02 * a.net
+    assert abs(float(a.w2()) / float(b.w2()) - 1) < 0.15
+    a.close(); b.close()
+
+
+@pytest.mark.parametrize("code,p,q", [(scheme(DEV_DTR, BLK_DB, 5), 1.0, 0.0), (scheme(DEV_DTR, BLK_DB, 5), 0.9, 0.1),
+                                      (scheme(DEV_DB, BLK_DT, 5), 1.0, 0.0)])
+def test_split_invariance(code, p, q):
+    a, b = Oracle(128, 3), Oracle(128, 3)
+    a.sweep(7, p, q, code)
+    b.sweep(3, p, q, code); b.sweep(0, p, q, code); b.sweep(4, p, q, code)
+    assert (a.lattice == b.lattice).all() and a.t == b.t == 7 and a.net == b.net
+    a.close(); b.close()
+
+
+@pytest.mark.parametrize("code,p,q", [(scheme(DEV_DTR, BLK_DB, 5), 1.0, 0.0), (scheme(DEV_DTR, BLK_DB, 5), 0.8, 0.3),
+                                      (scheme(DEV_DTR, BLK_DT, 5), 0.8, 0.3), (scheme(DEV_CDB, BLK_DB, 5), 1.0, 0.0)])
+def test_deposition_removal_symmetry(code, p, q):
+    """Mirror h -> -h exchanges minima and maxima, p and q, and complements every slope bit; the RNG
+    consumption does not depend on the state, so the two runs stay exact mirror images."""
+    a, b = Oracle(128, 13, init=0), Oracle(128, 13, init=1)
+    a.sweep(5, p, q, code)
+    b.sweep(5, q, p, code)
+    assert (a.lattice == ~b.lattice).all()
+    assert a.net == -b.net and a.h00 == -b.h00
+    assert (a.heights() == -b.heights()).all()
+    a.close(); b.close()
+
+
+def test_degenerate_sizes():
+    # L = 2D (a single tile) and D = cx (a single cell per domain)
+    for L, code in ((64, scheme(DEV_DTR, BLK_DB, 5)), (16, scheme(DEV_DTR, BLK_DB, 3)), (16, scheme(DEV_DB, BLK_DB, 4, 2, 2)),
+                    (16, scheme(DEV_DTR, BLK_DB, 3, 0, 0)), (16, scheme(DEV_DTR, BLK_DT, 3))):
+        o = Oracle(L, 2, track_heights=True)
+        o.sweep(5, 1.0, 0.0, code)
+        assert (o.heights() == o.tracked_heights).all()
+        assert o.net > 0
+        o.close()
+
+
+def test_invalid_schemes_are_rejected():
+    lib = oracle.lib()
+    assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DB, 7)) != 0        # L < 2D
+    assert lib.orc_check_scheme(128, scheme(DEV_DB, BLK_DB, 7)) == 0         # L >= D is enough for DB
+    assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DT, 5, 0, 1)) != 0  # DT needs TC >= 1,1 (:182)
+    assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DB, 3, 2, 0)) != 0  # cell larger than domain
+    assert lib.orc_check_scheme(96, scheme(DEV_DTR, BLK_DB, 4)) != 0         # L not a power of two
+    assert lib.orc_check_scheme(128, scheme(4, BLK_DB, 5)) != 0 and lib.orc_check_scheme(128, scheme(0, 3, 5)) != 0
+
+
+def test_filtered_run_reproduces_the_interior():
+    """A domain sweep depends only on its own (D+1)^2 window, so running only the domains that meet a
+    box reproduces the full run inside the box shrunk by 4(D+2) sites per MCS.  This is the tool the
+    full-size GPU parity tests use (L = 2^16, 2^17), validated here against complete runs."""
+    L, D, n = 512, 16, 2
+    code = scheme(DEV_DTR, BLK_DB, 4)
+    full = Oracle(L, 123)
+    full.sweep(n, 1.0, 0.0, code)
+    margin = n * 4 * (D + 2)
+    for (x0, y0, w, h) in ((40, 60, 200, 180), (L - 100, L - 90, 230, 210)):     # second box wraps
+        part = Oracle(L, 123)
+        part.set_filter(True, x0, y0, w, h)
+        part.sweep(n, 1.0, 0.0, code)
+        hf, hp = full.heights(), part.heights()
+        ys = (y0 + margin + np.arange(h - 2 * margin)) % L
+        xs = (x0 + margin + np.arange(w - 2 * margin)) % L
+        # compare slopes (heights differ by the anchor if (0,0) is outside the box)
+        sxf = hf - np.roll(hf, 1, axis=1); sxp = hp - np.roll(hp, 1, axis=1)
+        syf = hf - np.roll(hf, 1, axis=0); syp = hp - np.roll(hp, 1, axis=0)
+        assert (sxf[np.ix_(ys, xs)] == sxp[np.ix_(ys, xs)]).all()
+        assert (syf[np.ix_(ys, xs)] == syp[np.ix_(ys, xs)]).all()
+        assert (part.lattice != full.lattice).any()                               # and it really skipped work
+        part.close()
+    full.close()
