@@ -1,0 +1,140 @@
+/*
+ * oct.h -- C ABI of liboct_b200: the domain-decomposed (DD) random-sequential sweep of the 2+1-d
+ * octahedron model of arXiv 1705.01022 (Kelling, Odor, Gemming) on one NVIDIA B200 (sm_100a), with
+ * height reconstruction and the exact integer sums for W^2(t) and C_h(t,s).
+ *
+ * Citations are PAPER.md line numbers plus the section / equation they fall in; "R<n>" are the
+ * readings of silent or garbled passages listed in DESIGN.md.
+ *
+ * GENERAL RULES
+ *  - Every function returns OCT_OK (0) or a negative error code; nothing throws, aborts or prints.
+ *  - Pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  The caller owns every device
+ *    buffer and the stream; the library never allocates device memory.  `stream` is a cudaStream_t
+ *    passed as void* (NULL = the legacy default stream).
+ *  - Unless stated otherwise a call only ENQUEUES work on `stream` and returns; results land in
+ *    device buffers in stream order.  Calls that touch host buffers say whether they synchronise.
+ *  - The library runs on the current CUDA device and requires compute capability 10.x; there is no
+ *    CPU fallback: without a usable device every compute call returns OCT_ECUDA.
+ *  - Determinism: the lattice after oct_sweep depends only on (L, seed, init, the sequence of
+ *    (n_mcs, p, q, scheme)); never on grid size, timing or GPU model.  All randomness is counter-based
+ *    Philox4x32-10 keyed by (seed, mcs, set, domain, cell, step) (R19).
+ *
+ * DATA FORMATS
+ *  - Site (x,y), 0 <= x,y < L, periodic (:127).  sigma_x(x,y) = h(x,y)-h(x-1,y) and
+ *    sigma_y(x,y) = h(x,y)-h(x,y-1), each +-1, stored AT site (x,y) as one bit (1 <=> +1)  (:140, R2/R3).
+ *  - Packed lattice (:166, R4): L*L/4 bytes, little-endian uint32 words, word index wy*(L/4)+wx holds
+ *    the 4x4 sites (4wx+i, 4wy+j); sigma_x at bit 2(4j+i), sigma_y at bit 2(4j+i)+1.  This is both the
+ *    device layout and the exchange ("canonical") layout.
+ *  - Heights: int32, row-major [y*L + x].
+ */
+#ifndef OCT_B200_H
+#define OCT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct oct_ctx oct_ctx;   /* opaque host-side handle, owned by the library until oct_destroy */
+
+enum { OCT_OK = 0, OCT_EINVAL = -1, OCT_ECUDA = -2, OCT_ENOMEM = -3, OCT_ESTATE = -4 };
+
+enum {
+    OCT_INIT_FLAT = 0,          /* h = (x+y)&1: every word 0x33CC33CC, W^2 = 1/4 (R5)               */
+    OCT_INIT_FLAT_SHIFTED = 1,  /* h = -((x+y)&1): the bitwise complement, every word 0xCC33CC33     */
+    OCT_INIT_FROM_DEVICE = 2    /* the caller already filled lattice_dev (canonical words)          */
+};
+
+/* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16            (notation of Sec. 3.1.1 :176-182)
+ *   dev  (device layer, Sec. 3 :129-150):  0 DTr  double tiling with random origin   (:148-150)
+ *                                          1 DT   double tiling, fixed origin         (:142-146)
+ *                                          2 DB   dead border, free origin, width 5   (:133-140, :166)
+ *                                          3 cDB  dead border, origin on the 4-site grid, width 1 (:166)
+ *   blk  (block layer, single-hit, Sec. 3.1 :168-174):
+ *                                          0 DB   random cell origin per collective step; "ignoring
+ *                                                 borders" when only one of p,q is non-zero, delayed
+ *                                                 borders otherwise (:174, R16)
+ *                                          1 DB   delayed borders forced
+ *                                          2 DT   one random quadrant of every cell per step (:170)
+ *   tcx,tcy: log2 of the thread-cell edge in words of 4 sites, "TC=tcx,tcy" (:180); cell = 4<<tc sites
+ *   log2D  : log2 of the device-layer domain edge D in sites (the sub-tile one worker sweeps)       */
+#define OCT_SCHEME(dev, blk, tcx, tcy, log2D) \
+    ((dev) | ((blk) << 4) | ((tcx) << 8) | ((tcy) << 12) | ((log2D) << 16))
+enum { OCT_DEV_DTR = 0, OCT_DEV_DT = 1, OCT_DEV_DB = 2, OCT_DEV_CDB = 3 };
+enum { OCT_BLK_DB = 0, OCT_BLK_DB_DELAYED = 1, OCT_BLK_DT = 2 };
+
+/* Sizes of the caller-allocated device buffers for an L x L lattice (0 if L is invalid). */
+size_t oct_lattice_bytes(uint32_t L);      /* L*L/4                                                  */
+size_t oct_workspace_bytes(uint32_t L);    /* counters + two arrays of row anchors                   */
+
+/* Create a simulation on caller-owned device buffers (both 16-byte aligned).  Problem statement:
+ * Sec. 2.1 :25-34 (model), :127 (periodic, L x L).  L must be a power of two, 16 <= L <= 2^17.
+ * init = FLAT / FLAT_SHIFTED enqueue a fill of lattice_dev; FROM_DEVICE leaves it untouched.  The
+ * device counters (net deposits, tracked h(0,0)) are zeroed; the MCS clock starts at 0.
+ * Errors: EINVAL (bad L / init / null pointer), ECUDA (no sm_100 device, launch failure), ENOMEM. */
+int oct_create(oct_ctx** out, uint32_t L, uint64_t seed, int init,
+               void* lattice_dev, void* workspace_dev, void* stream);
+
+/* Overwrite the clock and the tracked anchors (used with INIT_FROM_DEVICE / oct_upload when the
+ * lattice is a continuation of an earlier run).  t < 2^32. */
+int oct_set_state(oct_ctx*, uint64_t t_mcs, int64_t h00, int64_t net, void* stream);
+
+/* n_mcs sweeps of the whole lattice (1 MCS = L^2 update attempts, :106) under DD scheme `scheme`,
+ * deposition probability p at local minima and removal probability q at local maxima (Eq. (1)
+ * :27-34; p,q in [0,1], quantised to 1/65536, R18).  DTr/DT: 4 kernel launches per MCS, one per domain
+ * set, in the permutation drawn for that MCS (:144); DB/cDB: 1 launch per MCS, and one such sweep
+ * lasts (1 - N_border/N) MCS of physical time (Eq. (9) :137, R9; see oct_time_per_sweep).
+ * oct_sweep(a) followed by oct_sweep(b) equals oct_sweep(a+b).
+ * Errors (nothing is enqueued): EINVAL for p,q outside [0,1], unknown dev/blk, cell larger than the
+ * domain, blk=DT with tc<1 (:182), L < 2D, D outside {32,64,128,256} or a (D,TC) pair the library was
+ * not built for, t+n_mcs > 2^32-1.  ECUDA: a launch failed (text via oct_last_error). */
+int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* stream);
+
+/* Integrate the slopes into int32 heights h[y*L+x] (:52 "peaks of the octahedra define the height
+ * profile"; anchor h(0,0) tracked exactly, R20).  heights_dev holds L*L int32. */
+int oct_heights(oct_ctx*, int32_t* heights_dev, void* stream);
+
+/* Integer sums for the roughness W^2(L,t) of Eq. (3) :61 (R6): out_dev[4] = {S1, S2, c, net} with
+ * c = h(0,0), S1 = sum (h-c), S2 = sum (h-c)^2 over all sites, net = deposits - removals so far.
+ * Exact as long as L^2 * max (h-c)^2 < 2^63. */
+int oct_width2(oct_ctx*, int64_t* out_dev, void* stream);
+
+/* Waiting-time snapshot for aging (:75-80): copies the packed lattice to lattice_copy_dev
+ * (oct_lattice_bytes) and writes anchor_out_dev[2] = {h(0,0), net} at this moment. */
+int oct_snapshot(oct_ctx*, void* lattice_copy_dev, int64_t* anchor_out_dev, void* stream);
+
+/* Integer sums for the height autocorrelation C_h(t,s) of Eq. (6) :92-98 (R7) between the current
+ * lattice and a snapshot: out_dev[5] = {S_t, S_s, S_ts, c_t, c_s}, S_t = sum (h_t-c_t),
+ * S_s = sum (h_s-c_s), S_ts = sum (h_t-c_t)(h_s-c_s).  With snapshot == current state the sums
+ * reproduce oct_width2's (C_h(s,s) = W^2(s), :97). */
+int oct_autocorr(oct_ctx*, const void* snapshot_dev, const int64_t* snapshot_anchor_dev,
+                 int64_t* out_dev, void* stream);
+
+/* Copy the packed lattice device -> host (canonical words).  SYNCHRONISES `stream`. */
+int oct_export(oct_ctx*, void* lattice_host, void* stream);
+/* Copy a packed lattice host -> device (enqueued; the host buffer must stay valid until the stream
+ * reaches the copy; pinned memory makes it asynchronous).  Anchors/clock are NOT changed. */
+int oct_upload(oct_ctx*, const void* lattice_host, void* stream);
+/* Read the device counters: out_host[2] = {h(0,0), net}.  SYNCHRONISES `stream`. */
+int oct_counters(oct_ctx*, int64_t* out_host, void* stream);
+
+int oct_mcs(const oct_ctx*, uint64_t* t_out);           /* sweeps done so far                        */
+int oct_destroy(oct_ctx*);                              /* frees the handle only (buffers are yours) */
+const char* oct_strerror(int code);
+const char* oct_last_error(const oct_ctx*);             /* text of the last CUDA failure, or ""     */
+
+/* Number of kernel launches the library has enqueued through this handle (for bench accounting). */
+int oct_launch_count(const oct_ctx*, uint64_t* n_out);
+
+/* Pure host helpers (no device work). */
+double oct_w2_from_sums(uint32_t L, int64_t S1, int64_t S2);                    /* (N*S2 - S1^2)/N^2  */
+double oct_c_from_sums(uint32_t L, int64_t St, int64_t Ss, int64_t Sts);        /* (N*Sts - St*Ss)/N^2 */
+double oct_time_per_sweep(uint32_t L, int scheme);   /* 1 for DT/DTr; (1 - N_border/N) for DB/cDB (R9) */
+int    oct_scheme_supported(uint32_t L, int scheme); /* OCT_OK or OCT_EINVAL, same checks as oct_sweep */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OCT_B200_H */

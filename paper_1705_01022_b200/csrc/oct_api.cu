@@ -1,0 +1,389 @@
+// liboct_b200: host side of the C ABI declared in include/oct.h.  Argument checking, launch
+// configuration and stream plumbing only -- every step of the hot path runs in the kernels of
+// sweep.cuh and observe.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include <cuda_runtime.h>
+
+#include "../../include/oct.h"
+#include "observe.cuh"
+#include "philox.cuh"
+#include "sweep.cuh"
+
+using namespace octb;
+
+struct oct_ctx {
+    uint32_t L = 0, log2L = 0;
+    uint64_t seed = 0;
+    uint64_t t = 0;
+    uint32_t* lat = nullptr;
+    unsigned char* ws = nullptr;
+    uint64_t launches = 0;
+    PhiloxRoundKeys rk{};
+    std::string last_error;
+
+    unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws); }
+    int32_t* anchorA() const { return reinterpret_cast<int32_t*>(ws + 256); }
+    int32_t* anchorB() const { return reinterpret_cast<int32_t*>(ws + 256 + (size_t)L * 4); }
+};
+
+namespace {
+
+constexpr uint32_t kMinL = 16, kMaxL = 1u << 17;
+
+bool valid_L(uint32_t L) { return L >= kMinL && L <= kMaxL && (L & (L - 1)) == 0; }
+
+uint32_t ilog2(uint32_t v) { uint32_t r = 0; while ((1u << r) < v) ++r; return r; }
+
+// probability -> 16-bit acceptance threshold, accept iff r16 < P16 (R18)
+uint32_t prob16(double p)
+{
+    const double v = p * 65536.0 + 0.5;
+    return v >= 65536.0 ? 65536u : static_cast<uint32_t>(v);
+}
+
+int fail_cuda(oct_ctx* c, cudaError_t e, const char* what)
+{
+    if (c) c->last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return OCT_ECUDA;
+}
+
+#define OCT_CUDA(ctx, call)                                         \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return fail_cuda(ctx, e__, #call);  \
+    } while (0)
+
+// ---- sweep kernel dispatch ---------------------------------------------------------------------------
+struct SweepLaunch {
+    void (*kern)(const SweepParams);
+    int threads, smem, dpb;
+};
+
+constexpr int pick_wpd(int log2d, int tcx, int tcy)
+{
+    const int ncell = ((1 << log2d) / (4 << tcx)) * ((1 << log2d) / (4 << tcy));
+    return ncell <= 256 ? 1 : ncell / 256;
+}
+
+template <int LD, int TX, int TY, int BLK>
+SweepLaunch make_launch()
+{
+    constexpr int W = pick_wpd(LD, TX, TY);
+    using SH = SweepShape<LD, TX, TY, W>;
+    return SweepLaunch{sweep_kernel<LD, TX, TY, BLK, W>, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
+}
+
+// (log2 D, tcx, tcy) combinations the library is built for
+#define OCT_SHAPES(X)                                                      \
+    X(5, 0, 0) X(5, 1, 1) X(5, 2, 2)                                       \
+    X(6, 0, 0) X(6, 1, 1) X(6, 2, 2) X(6, 2, 1) X(6, 3, 1) X(6, 1, 3)      \
+    X(7, 0, 0) X(7, 1, 1) X(7, 2, 2) X(7, 2, 1)                            \
+    X(8, 1, 1) X(8, 2, 2) X(8, 2, 1) X(8, 3, 2) X(8, 4, 1)
+
+bool find_launch(int ld, int tx, int ty, int blk, SweepLaunch* out)
+{
+#define X(LD, TX, TY)                                                               \
+    if (ld == LD && tx == TX && ty == TY) {                                         \
+        if (blk == kBlkSync) { *out = make_launch<LD, TX, TY, kBlkSync>(); return true; }       \
+        if (blk == kBlkDelayed) { *out = make_launch<LD, TX, TY, kBlkDelayed>(); return true; } \
+        if constexpr (TX >= 1 && TY >= 1) {                                         \
+            if (blk == kBlkDT) { *out = make_launch<LD, TX, TY, kBlkDT>(); return true; }       \
+        }                                                                           \
+        return false;                                                               \
+    }
+    OCT_SHAPES(X)
+#undef X
+    return false;
+}
+
+struct SchemeFields { uint32_t dev, blk, tcx, tcy, log2D; };
+
+SchemeFields split_scheme(int scheme)
+{
+    const uint32_t s = static_cast<uint32_t>(scheme);
+    return {s & 15u, (s >> 4) & 15u, (s >> 8) & 15u, (s >> 12) & 15u, (s >> 16) & 31u};
+}
+
+int check_scheme(uint32_t L, int scheme)
+{
+    if (scheme < 0 || !valid_L(L)) return OCT_EINVAL;
+    const SchemeFields f = split_scheme(scheme);
+    if ((static_cast<uint32_t>(scheme) >> 21) != 0) return OCT_EINVAL;
+    if (f.dev > 3 || f.blk > 2) return OCT_EINVAL;
+    if (f.log2D < 5 || f.log2D > 8) return OCT_EINVAL;
+    const uint32_t D = 1u << f.log2D, cx = 4u << f.tcx, cy = 4u << f.tcy;
+    if (cx > D || cy > D || cx > 64 || cy > 64) return OCT_EINVAL;
+    if (f.blk == OCT_BLK_DT && (f.tcx < 1 || f.tcy < 1)) return OCT_EINVAL;   // :182
+    if (L < 2 * D) return OCT_EINVAL;   // window (D/4+1 words) must not wrap onto itself
+    SweepLaunch sl;
+    if (!find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, f.blk == OCT_BLK_DT ? kBlkDT : kBlkSync, &sl)) return OCT_EINVAL;
+    return OCT_OK;
+}
+
+int ensure_device(oct_ctx* c)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(c, e, "cudaGetDevice");
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return fail_cuda(c, e, "cudaDeviceGetAttribute");
+    if (major != 10) {
+        if (c) c->last_error = "device is not compute capability 10.x (sm_100a build)";
+        return OCT_ECUDA;
+    }
+    return OCT_OK;
+}
+
+int launch_anchor(oct_ctx* c, const uint32_t* lat, int32_t* anchor, cudaStream_t st)
+{
+    column_anchor_kernel<<<1, kAnchorThreads, 0, st>>>(lat, c->L, anchor);
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t oct_lattice_bytes(uint32_t L) { return valid_L(L) ? (size_t)L * L / 4 : 0; }
+
+size_t oct_workspace_bytes(uint32_t L) { return valid_L(L) ? 256 + 2 * (size_t)L * sizeof(int32_t) : 0; }
+
+int oct_create(oct_ctx** out, uint32_t L, uint64_t seed, int init, void* lattice_dev, void* workspace_dev, void* stream)
+{
+    if (!out) return OCT_EINVAL;
+    *out = nullptr;
+    if (!valid_L(L) || !lattice_dev || !workspace_dev) return OCT_EINVAL;
+    if (init != OCT_INIT_FLAT && init != OCT_INIT_FLAT_SHIFTED && init != OCT_INIT_FROM_DEVICE) return OCT_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(lattice_dev) & 15u) || (reinterpret_cast<uintptr_t>(workspace_dev) & 15u)) return OCT_EINVAL;
+    oct_ctx* c = new (std::nothrow) oct_ctx;
+    if (!c) return OCT_ENOMEM;
+    c->L = L; c->log2L = ilog2(L); c->seed = seed; c->t = 0;
+    c->lat = static_cast<uint32_t*>(lattice_dev);
+    c->ws = static_cast<unsigned char*>(workspace_dev);
+    c->rk = make_round_keys(seed);
+    int rc = ensure_device(c);
+    if (rc != OCT_OK) { delete c; return rc; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemsetAsync(c->ws, 0, 256, st);
+    if (e == cudaSuccess && init != OCT_INIT_FROM_DEVICE) {
+        const size_t n_vec = (size_t)L * L / 4 / 16;
+        const unsigned blocks = (unsigned)((n_vec + 255) / 256 < 148 * 8 ? (n_vec + 255) / 256 : 148 * 8);
+        fill_words_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<uint4*>(c->lat), n_vec,
+                                                  init == OCT_INIT_FLAT ? 0x33CC33CCu : 0xCC33CC33u);
+        c->launches++;
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { delete c; return OCT_ECUDA; }
+    *out = c;
+    return OCT_OK;
+}
+
+int oct_set_state(oct_ctx* c, uint64_t t_mcs, int64_t h00, int64_t net, void* stream)
+{
+    if (!c || t_mcs > 0xFFFFFFFFull) return OCT_EINVAL;
+    set_counters_kernel<<<1, 1, 0, static_cast<cudaStream_t>(stream)>>>(c->counters(), h00, net);
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    c->t = t_mcs;
+    return OCT_OK;
+}
+
+int oct_scheme_supported(uint32_t L, int scheme) { return check_scheme(L, scheme); }
+
+int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* stream)
+{
+    if (!c) return OCT_EINVAL;
+    if (!(p >= 0.0 && p <= 1.0) || !(q >= 0.0 && q <= 1.0)) return OCT_EINVAL;
+    if (check_scheme(c->L, scheme) != OCT_OK) return OCT_EINVAL;
+    if (c->t + n_mcs > 0xFFFFFFFFull || c->t + n_mcs < c->t) return OCT_EINVAL;
+    const SchemeFields f = split_scheme(scheme);
+    const uint32_t P16 = prob16(p), Q16 = prob16(q);
+    const int blk = f.blk == OCT_BLK_DT ? kBlkDT
+                  : (f.blk == OCT_BLK_DB_DELAYED || (P16 > 0 && Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
+    SweepLaunch sl;
+    if (!find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &sl)) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (sl.smem > 48 * 1024)
+        OCT_CUDA(c, cudaFuncSetAttribute(sl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, sl.smem));
+
+    const bool tiled = f.dev <= OCT_DEV_DT;
+    const uint32_t nt = tiled ? c->L >> (f.log2D + 1) : c->L >> f.log2D;
+    const uint32_t ndom = nt * nt;
+    const uint32_t grid = (ndom + sl.dpb - 1) / sl.dpb;
+
+    SweepParams sp{};
+    sp.lat = c->lat; sp.counters = c->counters(); sp.L = c->L; sp.log2L = c->log2L;
+    sp.P16 = P16; sp.Q16 = Q16; sp.dev = f.dev; sp.ndom = ndom; sp.rk = c->rk;
+    for (uint64_t i = 0; i < n_mcs; ++i) {
+        sp.t = static_cast<uint32_t>(c->t);
+        for (uint32_t si = 0; si < (tiled ? 4u : 1u); ++si) {   // :144 sync = kernel boundary after each set
+            sp.si = si;
+            sl.kern<<<grid, sl.threads, sl.smem, st>>>(sp);
+            c->launches++;
+        }
+        OCT_CUDA(c, cudaGetLastError());
+        c->t++;
+    }
+    return OCT_OK;
+}
+
+int oct_heights(oct_ctx* c, int32_t* heights_dev, void* stream)
+{
+    if (!c || !heights_dev || (reinterpret_cast<uintptr_t>(heights_dev) & 15u)) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc = launch_anchor(c, c->lat, c->anchorA(), st);
+    if (rc) return rc;
+    RowsParams rp{};
+    rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters(); rp.heights = heights_dev; rp.L = c->L;
+    const uint32_t LW = c->L >> 2;
+    rows_kernel<kModeHeights><<<(LW + kRowsWarps - 1) / kRowsWarps, kRowsWarps * 32, 0, st>>>(rp);
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_width2(oct_ctx* c, int64_t* out_dev, void* stream)
+{
+    if (!c || !out_dev) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 4 * sizeof(int64_t), st));
+    int rc = launch_anchor(c, c->lat, c->anchorA(), st);
+    if (rc) return rc;
+    RowsParams rp{};
+    rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters();
+    rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
+    const uint32_t LW = c->L >> 2;
+    rows_kernel<kModeWidth2><<<(LW + kRowsWarps - 1) / kRowsWarps, kRowsWarps * 32, 0, st>>>(rp);
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_snapshot(oct_ctx* c, void* lattice_copy_dev, int64_t* anchor_out_dev, void* stream)
+{
+    if (!c || !lattice_copy_dev || !anchor_out_dev) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemcpyAsync(lattice_copy_dev, c->lat, oct_lattice_bytes(c->L), cudaMemcpyDeviceToDevice, st));
+    snapshot_anchor_kernel<<<1, 1, 0, st>>>(c->counters(), reinterpret_cast<long long*>(anchor_out_dev));
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_anchor_dev, int64_t* out_dev, void* stream)
+{
+    if (!c || !snapshot_dev || !snapshot_anchor_dev || !out_dev) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 5 * sizeof(int64_t), st));
+    int rc = launch_anchor(c, c->lat, c->anchorA(), st);
+    if (rc) return rc;
+    rc = launch_anchor(c, static_cast<const uint32_t*>(snapshot_dev), c->anchorB(), st);
+    if (rc) return rc;
+    RowsParams rp{};
+    rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
+    rp.anchorA = c->anchorA(); rp.anchorB = c->anchorB(); rp.countersA = c->counters();
+    rp.snapB = reinterpret_cast<const long long*>(snapshot_anchor_dev);
+    rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
+    const uint32_t LW = c->L >> 2;
+    rows_kernel<kModeAutocorr><<<(LW + kRowsWarps - 1) / kRowsWarps, kRowsWarps * 32, 0, st>>>(rp);
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_export(oct_ctx* c, void* lattice_host, void* stream)
+{
+    if (!c || !lattice_host) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemcpyAsync(lattice_host, c->lat, oct_lattice_bytes(c->L), cudaMemcpyDeviceToHost, st));
+    OCT_CUDA(c, cudaStreamSynchronize(st));
+    return OCT_OK;
+}
+
+int oct_upload(oct_ctx* c, const void* lattice_host, void* stream)
+{
+    if (!c || !lattice_host) return OCT_EINVAL;
+    OCT_CUDA(c, cudaMemcpyAsync(c->lat, lattice_host, oct_lattice_bytes(c->L), cudaMemcpyHostToDevice,
+                                static_cast<cudaStream_t>(stream)));
+    return OCT_OK;
+}
+
+int oct_counters(oct_ctx* c, int64_t* out_host, void* stream)
+{
+    if (!c || !out_host) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned long long tmp[2];
+    OCT_CUDA(c, cudaMemcpyAsync(tmp, c->counters(), sizeof(tmp), cudaMemcpyDeviceToHost, st));
+    OCT_CUDA(c, cudaStreamSynchronize(st));
+    out_host[0] = (int64_t)tmp[1];   // h(0,0)
+    out_host[1] = (int64_t)tmp[0];   // net
+    return OCT_OK;
+}
+
+int oct_mcs(const oct_ctx* c, uint64_t* t_out)
+{
+    if (!c || !t_out) return OCT_EINVAL;
+    *t_out = c->t;
+    return OCT_OK;
+}
+
+int oct_launch_count(const oct_ctx* c, uint64_t* n_out)
+{
+    if (!c || !n_out) return OCT_EINVAL;
+    *n_out = c->launches;
+    return OCT_OK;
+}
+
+int oct_destroy(oct_ctx* c)
+{
+    if (!c) return OCT_EINVAL;
+    delete c;
+    return OCT_OK;
+}
+
+const char* oct_strerror(int code)
+{
+    switch (code) {
+        case OCT_OK: return "ok";
+        case OCT_EINVAL: return "invalid argument";
+        case OCT_ECUDA: return "CUDA error (see oct_last_error)";
+        case OCT_ENOMEM: return "out of host memory";
+        case OCT_ESTATE: return "invalid state";
+        default: return "unknown error code";
+    }
+}
+
+const char* oct_last_error(const oct_ctx* c) { return c ? c->last_error.c_str() : ""; }
+
+double oct_w2_from_sums(uint32_t L, int64_t S1, int64_t S2)
+{
+    const __int128 N = (__int128)L * L;
+    const __int128 num = N * (__int128)S2 - (__int128)S1 * (__int128)S1;
+    return (double)((long double)num / ((long double)N * (long double)N));
+}
+
+double oct_c_from_sums(uint32_t L, int64_t St, int64_t Ss, int64_t Sts)
+{
+    const __int128 N = (__int128)L * L;
+    const __int128 num = N * (__int128)Sts - (__int128)St * (__int128)Ss;
+    return (double)((long double)num / ((long double)N * (long double)N));
+}
+
+double oct_time_per_sweep(uint32_t L, int scheme)
+{
+    if (check_scheme(L, scheme) != OCT_OK) return 0.0;
+    const SchemeFields f = split_scheme(scheme);
+    if (f.dev <= OCT_DEV_DT) return 1.0;
+    const double D = (double)(1u << f.log2D), w = f.dev == OCT_DEV_CDB ? 1.0 : 5.0;
+    return ((D - w) / D) * ((D - w) / D);   // Eq. (9) :137 with reading R9
+}
+
+}  // extern "C"

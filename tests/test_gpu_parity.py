@@ -1,0 +1,200 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit.
+
+Everything is integer work, so the bar is exact equality of lattice words, heights, counters and sums
+for the same (L, seed, init, scheme, p, q).  Sizes span one to many device-layer domains, several
+worker-group shapes, ragged word windows (random origins), wrap-around and the degenerate L = 2D.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import Oracle
+from paper_1705_01022_b200 import binding, workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def gpu_run(L, seed, code, n, p, q, init=wl.INIT_FLAT, chunks=None):
+    sim = binding.Sim(L, seed, init)
+    for c in (chunks or [n]):
+        sim.oct_sweep(c, p, q, code)
+    return sim
+
+
+def compare_state(sim, orc, check_heights=True):
+    words = sim.oct_export()
+    assert (words == orc.lattice).all(), f"{(words != orc.lattice).sum()} of {words.size} words differ"
+    h00, net = sim.oct_counters()
+    assert (h00, net) == (orc.h00, orc.net)
+    assert sim.oct_mcs() == orc.t
+    S = sim.oct_width2().cpu().numpy()
+    assert tuple(int(v) for v in S) == orc.sums()
+    if check_heights:
+        h = sim.oct_heights().cpu().numpy()
+        assert (h == orc.heights()).all()
+
+
+SMALL = [
+    # (L, code, p, q, n_mcs)
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 1.0, 0.0, 20),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 0.0, 1.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 0.9, 0.1, 12),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB_DELAYED, 6), 1.0, 0.0, 8),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6), 1.0, 0.0, 12),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6), 0.7, 0.3, 8),
+    (256, wl.scheme_code(wl.DEV_DT, wl.BLK_DB, 6), 1.0, 0.0, 8),
+    (256, wl.scheme_code(wl.DEV_DT, wl.BLK_DT, 6), 1.0, 0.0, 8),
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 8),
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DT, 6), 0.6, 0.4, 8),
+    (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 6), 1.0, 0.0, 8),
+    (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DT, 6), 1.0, 0.0, 8),
+    (64, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5), 1.0, 0.0, 16),               # L = 2D: a single tile
+    (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 5), 0.5, 0.5, 16),
+    (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 0, 0), 1.0, 0.0, 8),
+    (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 2, 2), 0.8, 0.2, 8),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 0, 0), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6, 2, 1), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 3, 1), 0.9, 0.1, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6, 1, 3), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 1.0, 0.0, 8),               # one warp, 8 cells per lane
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 0.9, 0.1, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 7), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 0, 0), 1.0, 0.0, 4),         # 4 warps per domain
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 2, 2), 0.9, 0.1, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 1.0, 0.0, 6),               # D = 256: 4 warps, named CTA barrier
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 0.9, 0.1, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 8), 1.0, 0.0, 4),
+    (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8), 1.0, 0.0, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8, 2, 2), 1.0, 0.0, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8, 3, 2), 0.9, 0.1, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 8, 4, 1), 1.0, 0.0, 4),
+]
+
+
+@pytest.mark.parametrize("L,code,p,q,n", SMALL, ids=[f"L{c[0]}-{wl.scheme_name(c[1])}-p{c[2]}q{c[3]}" for c in SMALL])
+def test_sweep_bit_exact(L, code, p, q, n):
+    seed = 1000 + L + (code & 0xFFFF)
+    orc = Oracle(L, seed)
+    orc.sweep(n, p, q, code)
+    sim = gpu_run(L, seed, code, n, p, q)
+    compare_state(sim, orc)
+    sim.close(); orc.close()
+
+
+def test_config0_L256_100mcs_per_mcs_sums():
+    """BASELINE config 1: L=256, D=64, p=1,q=0, 100 MCS, seed 1: lattice, heights and W^2(t) per MCS."""
+    cfg = wl.CONFIGS[0]
+    orc = Oracle(cfg.L, cfg.seeds[0])
+    sim = binding.Sim(cfg.L, cfg.seeds[0])
+    for t in range(cfg.n_mcs):
+        orc.sweep(1, cfg.p, cfg.q, cfg.scheme)
+        sim.oct_sweep(1, cfg.p, cfg.q, cfg.scheme)
+        S = tuple(int(v) for v in sim.oct_width2().cpu().numpy())
+        assert S == orc.sums(), t
+        assert binding.oct_w2_from_sums(cfg.L, S[0], S[1]) == pytest.approx(float(orc.w2()), rel=1e-14)
+    compare_state(sim, orc)
+    sim.close(); orc.close()
+
+
+def test_split_invariance_and_resume():
+    L, code = 256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6)
+    a = gpu_run(L, 5, code, 9, 1.0, 0.0)
+    b = gpu_run(L, 5, code, 9, 1.0, 0.0, chunks=[2, 0, 3, 4])
+    assert (a.oct_export() == b.oct_export()).all() and a.oct_counters() == b.oct_counters()
+    # resume from an exported lattice on a fresh handle
+    words = a.oct_export()
+    h00, net = a.oct_counters()
+    c = binding.Sim(L, 5, wl.INIT_FROM_DEVICE, lattice=torch.from_numpy(words.view(np.int32).reshape(-1)).cuda())
+    c.oct_set_state(9, h00, net)
+    a.oct_sweep(3, 1.0, 0.0, code); c.oct_sweep(3, 1.0, 0.0, code)
+    assert (a.oct_export() == c.oct_export()).all() and a.oct_counters() == c.oct_counters()
+    orc = Oracle(L, 5); orc.sweep(12, 1.0, 0.0, code)
+    compare_state(c, orc)
+    for s in (a, b, c):
+        s.close()
+    orc.close()
+
+
+def test_flat_shifted_symmetry_on_gpu():
+    L, code = 256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6)
+    a = gpu_run(L, 3, code, 5, 0.8, 0.3, init=wl.INIT_FLAT)
+    b = gpu_run(L, 3, code, 5, 0.3, 0.8, init=wl.INIT_FLAT_SHIFTED)
+    assert (a.oct_export() == ~b.oct_export()).all()
+    ha, na = a.oct_counters(); hb, nb = b.oct_counters()
+    assert (ha, na) == (-hb, -nb)
+    orc = Oracle(L, 3, init=1); orc.sweep(5, 0.3, 0.8, code)
+    compare_state(b, orc)
+    a.close(); b.close(); orc.close()
+
+
+@pytest.mark.parametrize("L,seed,off", [(16, 1, 0), (64, 2, -7), (128, 5, 3), (256, 3, 1000), (1024, 4, -123456)])
+def test_heights_and_sums_on_synthetic_surfaces(L, seed, off):
+    """Reconstruction / reduction kernels on surfaces unrelated to the dynamics (rough, ragged L)."""
+    h = wl.separable_surface(L, seed, off)
+    words = wl.pack_heights(h)
+    sim = binding.Sim(L, 0, wl.INIT_FROM_DEVICE, lattice=torch.from_numpy(words.view(np.int32).reshape(-1)).cuda())
+    sim.oct_set_state(0, off, 17)
+    orc = Oracle(L, 0); orc.set_lattice(words, h00=off, net=17)
+    assert (sim.oct_heights().cpu().numpy() == h).all()
+    assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == orc.sums()
+    # autocorrelation against a second, different surface
+    h2 = wl.separable_surface(L, seed + 100, off - 5)
+    snap = torch.from_numpy(wl.pack_heights(h2).view(np.int32).reshape(-1)).cuda()
+    anchor = torch.tensor([off - 5, 3], dtype=torch.int64, device="cuda")
+    got = tuple(int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy())
+    orc2 = Oracle(L, 0); orc2.set_lattice(wl.pack_heights(h2), h00=off - 5, net=3)
+    assert got == orc.autocorr_sums(orc2)
+    sim.close(); orc.close(); orc2.close()
+
+
+def test_aging_snapshot_and_autocorrelation():
+    L, code = 256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6)
+    orc = Oracle(L, 8); sim = binding.Sim(L, 8)
+    orc.sweep(10, 1.0, 0.0, code); sim.oct_sweep(10, 1.0, 0.0, code)
+    osnap = orc.clone()
+    snap, anchor = sim.oct_snapshot()
+    # C_h(s,s) sums reproduce the W^2 sums
+    S = [int(v) for v in sim.oct_width2().cpu().numpy()]
+    A = [int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy()]
+    assert A[0] == A[1] == S[0] and A[2] == S[1] and A[3] == A[4] == S[2]
+    for n in (5, 15):
+        orc.sweep(n, 1.0, 0.0, code); sim.oct_sweep(n, 1.0, 0.0, code)
+        A = tuple(int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy())
+        assert A == orc.autocorr_sums(osnap)
+        assert binding.oct_c_from_sums(L, A[0], A[1], A[2]) == pytest.approx(float(orc.c_h(osnap)), rel=1e-13)
+    sim.close(); orc.close(); osnap.close()
+
+
+def test_config1_shape_all_schemes_L1024_prefix():
+    """BASELINE config 2 (L=1024, D=128, every device-layer scheme): first MCS bit-exact per scheme."""
+    L = 1024
+    for code in wl.ALL_SCHEMES(7):
+        orc = Oracle(L, 2); sim = binding.Sim(L, 2)
+        orc.sweep(3, 1.0, 0.0, code); sim.oct_sweep(3, 1.0, 0.0, code)
+        compare_state(sim, orc, check_heights=False)
+        sim.close(); orc.close()
+
+
+def test_config2_shape_mixed_rates_L4096_prefix():
+    """BASELINE config 3 (L=4096, p=0.9, q=0.1, seed 7, D=128, delayed borders): first 2 MCS."""
+    cfg = wl.CONFIGS[2]
+    orc = Oracle(cfg.L, cfg.seeds[0]); sim = binding.Sim(cfg.L, cfg.seeds[0])
+    orc.sweep(2, cfg.p, cfg.q, cfg.scheme); sim.oct_sweep(2, cfg.p, cfg.q, cfg.scheme)
+    compare_state(sim, orc, check_heights=False)
+    sim.close(); orc.close()
+
+
+def test_invalid_calls_are_rejected_without_side_effects():
+    sim = binding.Sim(256, 1)
+    before = sim.oct_export().copy()
+    for args in ((1, 1.5, 0.0, wl.scheme_code(0, 0, 6)), (1, 1.0, -0.1, wl.scheme_code(0, 0, 6)),
+                 (1, 1.0, 0.0, wl.scheme_code(0, 0, 8)), (1, 1.0, 0.0, wl.scheme_code(0, 2, 6, 0, 0)),
+                 (1 << 33, 1.0, 0.0, wl.scheme_code(0, 0, 6))):
+        with pytest.raises(binding.OctError) as e:
+            sim.oct_sweep(*args)
+        assert e.value.code == binding.OCT_EINVAL
+    assert (sim.oct_export() == before).all() and sim.oct_mcs() == 0
+    sim.close()
