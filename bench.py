@@ -153,6 +153,7 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--ref-L", type=int, default=4096, help="lattice edge of the oracle's timed sample")
     ap.add_argument("--ref-mcs", type=int, default=32)
+    ap.add_argument("--kernel", type=int, default=0, help="OCT_OPT_KERNEL value: 0 auto, 1 bit-packed, 2 link-entry variant B")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -181,6 +182,7 @@ def main():
     code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, args.log2D)
     seed = wl.rank_seed(args.seed, rank)
     sim = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
+    sim.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)
     stream = torch.cuda.current_stream()
     sim.oct_sweep(args.burn_in, 1.0, 0.0, code)            # evolved state: acceptance ~0.17 (not the flat 0.5)
     snap, anchor = sim.oct_snapshot()

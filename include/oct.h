@@ -125,6 +125,15 @@ int oct_destroy(oct_ctx*);                              /* frees the handle only
 const char* oct_strerror(int code);
 const char* oct_last_error(const oct_ctx*);             /* text of the last CUDA failure, or ""     */
 
+/* Implementation options.  They never change results (every kernel is bit-identical to the oracle), only
+ * which kernel runs.  OCT_OPT_KERNEL: AUTO picks the link-entry kernel (one 32-bit entry of four link
+ * bytes per site in shared memory, no atomics) for DTr/DT with D <= 128 and the bit-packed kernel
+ * otherwise; BITPACKED forces the latter; LINKS_B selects the alternative work split (fewer warps per
+ * domain, two cells per lane) where one is built.  EINVAL for unknown options / values. */
+enum { OCT_OPT_KERNEL = 1 };
+enum { OCT_KERNEL_AUTO = 0, OCT_KERNEL_BITPACKED = 1, OCT_KERNEL_LINKS_B = 2 };
+int oct_set_option(oct_ctx*, int option, int value);
+
 /* Number of kernel launches the library has enqueued through this handle (for bench accounting). */
 int oct_launch_count(const oct_ctx*, uint64_t* n_out);
 

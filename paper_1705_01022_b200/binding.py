@@ -21,8 +21,10 @@ EXPORTS = (
     "oct_lattice_bytes", "oct_workspace_bytes", "oct_create", "oct_set_state", "oct_sweep", "oct_heights",
     "oct_width2", "oct_snapshot", "oct_autocorr", "oct_export", "oct_upload", "oct_counters", "oct_mcs",
     "oct_destroy", "oct_strerror", "oct_last_error", "oct_launch_count", "oct_w2_from_sums", "oct_c_from_sums",
-    "oct_time_per_sweep", "oct_scheme_supported",
+    "oct_time_per_sweep", "oct_scheme_supported", "oct_set_option",
 )
+OCT_OPT_KERNEL = 1
+OCT_KERNEL_AUTO, OCT_KERNEL_BITPACKED, OCT_KERNEL_LINKS_B = 0, 1, 2
 
 
 class OctError(RuntimeError):
@@ -62,6 +64,7 @@ def load(rebuild_if_stale: bool = True):
         "oct_launch_count": (i32, [vp, C.POINTER(u64)]),
         "oct_w2_from_sums": (dbl, [u32, i64, i64]), "oct_c_from_sums": (dbl, [u32, i64, i64, i64]),
         "oct_time_per_sweep": (dbl, [u32, i32]), "oct_scheme_supported": (i32, [u32, i32]),
+        "oct_set_option": (i32, [vp, i32, i32]),
     }
     for name in EXPORTS:
         fn = getattr(L, name)          # AttributeError if a declared symbol is not exported
@@ -212,6 +215,9 @@ class Sim:
         o = np.zeros(2, dtype=np.int64)
         self._check(self._l.oct_counters(self._h, o.ctypes.data, _stream_ptr(stream)), "oct_counters")
         return int(o[0]), int(o[1])
+
+    def oct_set_option(self, option: int, value: int):
+        self._check(self._l.oct_set_option(self._h, option, value), "oct_set_option")
 
     def oct_mcs(self) -> int:
         t = C.c_uint64()

@@ -13,6 +13,7 @@
 #include "observe.cuh"
 #include "philox.cuh"
 #include "sweep.cuh"
+#include "sweep_links.cuh"
 
 using namespace octb;
 
@@ -23,6 +24,7 @@ struct oct_ctx {
     uint32_t* lat = nullptr;
     unsigned char* ws = nullptr;
     uint64_t launches = 0;
+    int opt_kernel = OCT_KERNEL_AUTO;
     PhiloxRoundKeys rk{};
     std::string last_error;
 
@@ -97,6 +99,38 @@ bool find_launch(int ld, int tx, int ty, int blk, SweepLaunch* out)
         return false;                                                               \
     }
     OCT_SHAPES(X)
+#undef X
+    return false;
+}
+
+// ---- link-entry sweep kernel (sweep_links.cuh): DTr/DT device layer, D <= 128 ------------------------
+template <int LD, int TX, int TY, int BLK, int W, int DPB>
+SweepLaunch make_links_launch()
+{
+    using SH = LinkShape<LD, TX, TY, W, DPB>;
+    return SweepLaunch{sweep_links_kernel<LD, TX, TY, BLK, W, DPB>, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
+}
+
+// (log2 D, tcx, tcy, warps per domain, domains per CTA): variant A is the default, variant B the
+// alternative work split of the two headline shapes (fewer warps, two cells per lane)
+#define OCT_LINK_SHAPES_A(X)                                                         \
+    X(5, 0, 0, 1, 4) X(6, 0, 0, 4, 1) X(6, 1, 1, 2, 2) X(6, 2, 1, 1, 4)              \
+    X(7, 0, 0, 8, 1) X(7, 1, 1, 8, 1) X(7, 2, 2, 2, 1) X(7, 2, 1, 4, 1)
+#define OCT_LINK_SHAPES_B(X) X(6, 1, 1, 1, 4) X(7, 1, 1, 4, 1)
+
+bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, SweepLaunch* out)
+{
+#define X(LD, TX, TY, W, DPB)                                                                        \
+    if (ld == LD && tx == TX && ty == TY) {                                                          \
+        if (blk == kBlkSync) { *out = make_links_launch<LD, TX, TY, kBlkSync, W, DPB>(); return true; }       \
+        if (blk == kBlkDelayed) { *out = make_links_launch<LD, TX, TY, kBlkDelayed, W, DPB>(); return true; } \
+        if constexpr (TX >= 1 && TY >= 1) {                                                          \
+            if (blk == kBlkDT) { *out = make_links_launch<LD, TX, TY, kBlkDT, W, DPB>(); return true; }       \
+        }                                                                                            \
+        return false;                                                                                \
+    }
+    if (variant_b) { OCT_LINK_SHAPES_B(X) }
+    OCT_LINK_SHAPES_A(X)
 #undef X
     return false;
 }
@@ -198,6 +232,13 @@ int oct_set_state(oct_ctx* c, uint64_t t_mcs, int64_t h00, int64_t net, void* st
 
 int oct_scheme_supported(uint32_t L, int scheme) { return check_scheme(L, scheme); }
 
+int oct_set_option(oct_ctx* c, int option, int value)
+{
+    if (!c) return OCT_EINVAL;
+    if (option == OCT_OPT_KERNEL && value >= OCT_KERNEL_AUTO && value <= OCT_KERNEL_LINKS_B) { c->opt_kernel = value; return OCT_OK; }
+    return OCT_EINVAL;
+}
+
 int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* stream)
 {
     if (!c) return OCT_EINVAL;
@@ -209,7 +250,11 @@ int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* 
     const int blk = f.blk == OCT_BLK_DT ? kBlkDT
                   : (f.blk == OCT_BLK_DB_DELAYED || (P16 > 0 && Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
     SweepLaunch sl;
-    if (!find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &sl)) return OCT_EINVAL;
+    // the link-entry kernel serves the tiled device layers on domains that fit shared memory unpacked;
+    // the bit-packed kernel serves everything else (D = 256, dead-border device layers, tiny domains)
+    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED && f.dev <= OCT_DEV_DT &&
+                       find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B, &sl);
+    if (!links && !find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &sl)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (sl.smem > 48 * 1024)
         OCT_CUDA(c, cudaFuncSetAttribute(sl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, sl.smem));

@@ -16,8 +16,9 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 
-def gpu_run(L, seed, code, n, p, q, init=wl.INIT_FLAT, chunks=None):
+def gpu_run(L, seed, code, n, p, q, init=wl.INIT_FLAT, chunks=None, kernel=binding.OCT_KERNEL_AUTO):
     sim = binding.Sim(L, seed, init)
+    sim.oct_set_option(binding.OCT_OPT_KERNEL, kernel)
     for c in (chunks or [n]):
         sim.oct_sweep(c, p, q, code)
     return sim
@@ -74,14 +75,36 @@ SMALL = [
 ]
 
 
+KERNELS = {"auto": binding.OCT_KERNEL_AUTO, "bitpacked": binding.OCT_KERNEL_BITPACKED, "linksB": binding.OCT_KERNEL_LINKS_B}
+
+
 @pytest.mark.parametrize("L,code,p,q,n", SMALL, ids=[f"L{c[0]}-{wl.scheme_name(c[1])}-p{c[2]}q{c[3]}" for c in SMALL])
 def test_sweep_bit_exact(L, code, p, q, n):
+    """Every kernel the library can pick for a scheme (link-entry, its alternative work split, bit-packed)
+    gives the oracle's lattice, counters, sums and heights."""
     seed = 1000 + L + (code & 0xFFFF)
     orc = Oracle(L, seed)
     orc.sweep(n, p, q, code)
-    sim = gpu_run(L, seed, code, n, p, q)
-    compare_state(sim, orc)
-    sim.close(); orc.close()
+    for name, k in KERNELS.items():
+        sim = gpu_run(L, seed, code, n, p, q, kernel=k)
+        compare_state(sim, orc, check_heights=(name == "auto"))
+        sim.close()
+    orc.close()
+
+
+def test_origin_site_height_is_tracked_when_it_is_updated():
+    """The tracked anchor h(0,0) (R20) moves only when site (0,0) itself is updated: long enough runs on a
+    small lattice that it moves many times, both directions, all kernels."""
+    L = 64
+    for code, p, q in ((wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 0, 0), 1.0, 0.0), (wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 0, 0), 0.0, 1.0),
+                       (wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 0, 0), 0.6, 0.4), (wl.scheme_code(wl.DEV_DT, wl.BLK_DT, 5, 1, 1), 0.7, 0.2)):
+        orc = Oracle(L, 77); orc.sweep(60, p, q, code)
+        assert orc.h00 != 0
+        for k in KERNELS.values():
+            sim = gpu_run(L, 77, code, 60, p, q, kernel=k)
+            compare_state(sim, orc, check_heights=False)
+            sim.close()
+        orc.close()
 
 
 def test_config0_L256_100mcs_per_mcs_sums():
