@@ -29,9 +29,10 @@ sys.path.insert(0, ROOT)
 METRIC = "site_update_attempts_per_s"
 UNIT = "attempts/s"
 
-# Algorithmic lane-instructions per update attempt of the DTrDB sync sweep (DESIGN.md "Roofline of the
-# sweep kernel"): Philox 42/4 + decode 11 + loads/tests 12 + apply (17 % of attempts) 3 + loop/sync 3.
-I_ALG = 40.0
+# Algorithmic lane-instructions per update attempt of the DTrDB sweep in the link-entry design (DESIGN.md
+# section 6): Philox4x32-10 40/4 = 10, site select 5, entry load + compare 2, five stores of an accepted
+# update (issued warp-wide) 5, step loop/sync 1, staging (expand + gather + moments per site) 9.
+I_ALG = 32.0
 # the paper's DTrDB throughput at L = 2^16, p=1, q=0 on Kepler GPUs, per GPU
 PAPER_ATTEMPTS_PER_S = 9.0e9
 N_SM, SMSP, LANES = 148, 4, 32
@@ -147,7 +148,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=1 << 16)
-    ap.add_argument("--log2D", type=int, default=8)
+    ap.add_argument("--log2D", type=int, default=6)
     ap.add_argument("--mcs-per-step", type=int, default=8)
     ap.add_argument("--burn-in", type=int, default=32)
     ap.add_argument("--seed", type=int, default=1)
@@ -249,9 +250,9 @@ def main():
         except Exception:
             traffic = None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-instr/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": "sweep_kernel", "avg_launch_ms": launch_s * 1e3, "instr_per_attempt": I_ALG,
+                "traffic": traffic, "kernel": "sweep_links_kernel" if (args.log2D <= 7 and args.kernel != 1) else "sweep_kernel", "avg_launch_ms": launch_s * 1e3, "instr_per_attempt": I_ALG,
                 "peak_src": f"148 SM x 4 SMSP x 32 lanes x sm_max_mhz ({peaks['src']})",
-                "hbm_gbs_of_sweep": 0.5 * 1.0317 * attempts_per_launch / launch_s / 1e9,
+                "hbm_gbs_of_sweep": 0.5 * (1.0 + 4.0 / (1 << args.log2D)) ** 2 * attempts_per_launch / launch_s / 1e9,
                 "sweep_share_of_step": sweep_ms / total_ms}
 
     # ---- e2e: same step through the C ABI with HOST buffers ------------------------------------------

@@ -111,12 +111,13 @@ SweepLaunch make_links_launch()
     return SweepLaunch{sweep_links_kernel<LD, TX, TY, BLK, W, DPB>, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
 }
 
-// (log2 D, tcx, tcy, warps per domain, domains per CTA): variant A is the default, variant B the
-// alternative work split of the two headline shapes (fewer warps, two cells per lane)
+// (log2 D, tcx, tcy, warps per domain, domains per CTA): variant A is the default (the faster one on
+// B200: D=64 one warp per domain, two cells per lane, warp-level sync only; D=128 eight warps), variant
+// B the alternative work split of the two headline shapes
 #define OCT_LINK_SHAPES_A(X)                                                         \
-    X(5, 0, 0, 1, 4) X(6, 0, 0, 4, 1) X(6, 1, 1, 2, 2) X(6, 2, 1, 1, 4)              \
+    X(5, 0, 0, 1, 4) X(6, 0, 0, 4, 1) X(6, 1, 1, 1, 4) X(6, 2, 1, 1, 4)              \
     X(7, 0, 0, 8, 1) X(7, 1, 1, 8, 1) X(7, 2, 2, 2, 1) X(7, 2, 1, 4, 1)
-#define OCT_LINK_SHAPES_B(X) X(6, 1, 1, 1, 4) X(7, 1, 1, 4, 1)
+#define OCT_LINK_SHAPES_B(X) X(6, 1, 1, 2, 2) X(7, 1, 1, 4, 1)
 
 bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, SweepLaunch* out)
 {

@@ -96,6 +96,26 @@ __device__ __forceinline__ uint32_t gather_word(const uint32_t* __restrict__ S, 
     return word;
 }
 
+// entry index y*P + x of the site packed as v = x | y << 8 (fields may hold x + D, y + D: cells wrap inside
+// the domain, R14): mask both fields at once, then y*P + x = vm + y*(P - 256)
+template <class SH>
+__device__ __forceinline__ uint32_t site_index(uint32_t v)
+{
+    const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
+    return (vm >> 8) * (uint32_t)(SH::P - 256) + vm;
+}
+
+// First moment sum_x x * b(x) of the sigma_x bits of packed window word (iw, .), x = 4*iw + i.  The sweep
+// does not count its accepted updates: inside a window row the heights of the sites west and east of the
+// active span are fixed during the launch, so sum_x delta b(x) = 0 and the rise of the surface is
+// sum_sites delta h = -2 sum x * delta b(x); every deposit raises one site by 2, hence
+//     deposits - removals = sum over window words of (moment before - moment after).
+__device__ __forceinline__ int x_moment(uint32_t word, uint32_t iw)
+{
+    const uint32_t m = word & 0x55555555u;
+    return (int)(4u * iw * __popc(m) + __popc(m & 0x44444444u) + 2u * __popc(m & 0x50505050u));
+}
+
 // Carry out an accepted update at entry index `i` (relative to Sb): the site's four links flip.
 // up = true: deposition (minimum -> maximum), false: removal.
 template <class SH>
@@ -110,11 +130,10 @@ __device__ __forceinline__ void flip_links(uint32_t* Sb, uint32_t i, bool up)
     B[+4 * SH::P + 2] = v0;         // north neighbour's S link = sigma_y(x,y+1)
 }
 
-// The collective single-hit steps of one domain sweep (:168-174).  Returns deposits minus removals of
-// this thread.  ALWAYS: the acceptance threshold of the only live direction is 65536 (p = 1 or q = 1),
+// The collective single-hit steps of one domain sweep (:168-174).  ALWAYS: the acceptance threshold of the only live direction is 65536 (p = 1 or q = 1),
 // so the r16 comparison is dropped.
 template <class SH, int BLK, bool ALWAYS>
-__device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32_t* __restrict__ BT, uint32_t tg, int grp,
+__device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint32_t* __restrict__ BT, uint32_t tg, int grp,
                                          uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16)
 {
     constexpr int CX = SH::CX, CY = SH::CY, D = SH::D, G = SH::G, CPT = SH::CPT;
@@ -133,7 +152,6 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32
     // sync variant: exactly one direction is live (p*q == 0)
     const bool dep = Q16 == 0u;
     const uint32_t target = dep ? kEntryMin : kEntryMax, T16 = dep ? P16 : Q16;
-    int cnt = 0;
 
 #pragma unroll 1
     for (uint32_t k4 = 0; k4 < (uint32_t)(SH::NSTEP / 4); ++k4) {
@@ -141,9 +159,11 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32
 #pragma unroll
         for (int j = 0; j < CPT; ++j) philox4x32_10(k4, tg + j * G, c2c, t, rk, rw[j]);
 
+        const uint4 bq = *reinterpret_cast<const uint4*>(BT + 4 * k4);   // one broadcast load for four steps
+        const uint32_t bw4[4] = {bq.x, bq.y, bq.z, bq.w};
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
-            const uint32_t Bw = BT[4 * k4 + kk];
+            const uint32_t Bw = bw4[kk];
             uint32_t idx[CPT];
             if constexpr (BLK == kBlkSync) {
                 // "ignoring borders" (:174) made order-free (R16): all cells decide on the state at the start
@@ -154,14 +174,14 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
                     const uint32_t v = (w & FM) + cellc[j] + sc;
-                    idx[j] = ((v >> 8) & (D - 1)) * SH::P + (v & (D - 1));
+                    idx[j] = site_index<SH>(v);
                     acc[j] = Sb[idx[j]] == target;
                     if constexpr (!ALWAYS) acc[j] = acc[j] && (w >> 16) < T16;
                 }
                 group_sync<SH::WPD, SH::DPB>(grp);
 #pragma unroll
                 for (int j = 0; j < CPT; ++j)
-                    if (acc[j]) { flip_links<SH>(Sb, idx[j], dep); ++cnt; }
+                    if (acc[j]) flip_links<SH>(Sb, idx[j], dep);
                 group_sync<SH::WPD, SH::DPB>(grp);
             } else if constexpr (BLK == kBlkDelayed) {
                 // delayed borders (:174): bulk, then edges, then corners (R15)
@@ -171,7 +191,7 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t f = rw[j][kk] & FM;
                     const uint32_t v = f + cellc[j] + sc;
-                    idx[j] = ((v >> 8) & (D - 1)) * SH::P + (v & (D - 1));
+                    idx[j] = site_index<SH>(v);
                     cls[j] = (uint32_t)((f & 0xFFu) == (uint32_t)(CX - 1)) + (uint32_t)((f >> 8) == (uint32_t)(CY - 1));
                 }
 #pragma unroll
@@ -180,8 +200,8 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32
                     for (int j = 0; j < CPT; ++j)
                         if (cls[j] == phase) {
                             const uint32_t e = Sb[idx[j]], r16 = rw[j][kk] >> 16;
-                            if (e == kEntryMin && r16 < P16) { flip_links<SH>(Sb, idx[j], true); ++cnt; }
-                            else if (e == kEntryMax && r16 < Q16) { flip_links<SH>(Sb, idx[j], false); --cnt; }
+                            if (e == kEntryMin && r16 < P16) flip_links<SH>(Sb, idx[j], true);
+                            else if (e == kEntryMax && r16 < Q16) flip_links<SH>(Sb, idx[j], false);
                         }
                     group_sync<SH::WPD, SH::DPB>(grp);
                 }
@@ -192,17 +212,15 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ Sb, const uint32
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
                     const uint32_t v = (w & FM) + cellc[j] + qc;
-                    const uint32_t i = ((v >> 8) & (D - 1)) * SH::P + (v & (D - 1));
+                    const uint32_t i = site_index<SH>(v);
                     const uint32_t e = Sb[i], r16 = w >> 16;
-                    if (e == kEntryMin && r16 < P16) { flip_links<SH>(Sb, i, true); ++cnt; }
-                    else if (e == kEntryMax && r16 < Q16) { flip_links<SH>(Sb, i, false); --cnt; }
+                    if (e == kEntryMin && r16 < P16) flip_links<SH>(Sb, i, true);
+                    else if (e == kEntryMax && r16 < Q16) flip_links<SH>(Sb, i, false);
                 }
                 group_sync<SH::WPD, SH::DPB>(grp);
             }
         }
     }
-    if constexpr (BLK == kBlkSync) return dep ? cnt : -cnt;
-    else return cnt;
 }
 
 // number of set W links of the sites (0..x00, y00) of the domain: h(x00,y00) minus the height of the
@@ -247,11 +265,29 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
     uint32_t* Sb = S + offy * SH::P + offx;          // entry of the domain's site (0,0)
 
     // ---- a2: stage-in (:164): packed words -> link entries -------------------------------------
-    for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
-        const uint32_t jw = idx / NW, iw = idx - jw * NW;
-        const size_t r0 = (size_t)((wy0 + jw) & LWm) * LW, r1 = (size_t)((wy0 + jw + 1u) & LWm) * LW;
-        const uint32_t c0 = (wx0 + iw) & LWm, c1 = (wx0 + iw + 1u) & LWm;
-        expand_word<SH>(S, iw, jw, P.lat[r0 + c0], P.lat[r0 + c1], P.lat[r1 + c0]);
+    int net = 0;                                     // deposits - removals, from the x-moments (see x_moment)
+    {
+        constexpr int NIT = (NW * NW + G - 1) / G;   // words per thread; all loads are issued before the first use
+        uint32_t A[NIT], Ew[NIT], Nw[NIT];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const uint32_t idx = tg + it * G;
+            if (idx < (uint32_t)(NW * NW)) {
+                const uint32_t jw = idx / NW, iw = idx - jw * NW;
+                const size_t r0 = (size_t)((wy0 + jw) & LWm) * LW, r1 = (size_t)((wy0 + jw + 1u) & LWm) * LW;
+                const uint32_t c0 = (wx0 + iw) & LWm, c1 = (wx0 + iw + 1u) & LWm;
+                A[it] = P.lat[r0 + c0]; Ew[it] = P.lat[r0 + c1]; Nw[it] = P.lat[r1 + c0];
+            }
+        }
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const uint32_t idx = tg + it * G;
+            if (idx < (uint32_t)(NW * NW)) {
+                const uint32_t jw = idx / NW, iw = idx - jw * NW;
+                expand_word<SH>(S, iw, jw, A[it], Ew[it], Nw[it]);
+                net += x_moment(A[it], iw);
+            }
+        }
     }
     // ---- a3: block-step table (:170, :172; R13/R17/R24) ----------------------------------------
     const uint32_t c2b = (kTagBlock << 30) | (set << 28) | dom, c2c = (kTagCell << 30) | (set << 28) | dom;
@@ -272,20 +308,21 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
     }
 
     // ---- a4-a6: collective single-hit steps (:168) ---------------------------------------------
-    int net;
     if constexpr (BLK == kBlkSync) {
         const uint32_t T16 = P.Q16 == 0u ? P.P16 : P.Q16;
-        if (T16 == 65536u) net = run_steps<SH, BLK, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
-        else               net = run_steps<SH, BLK, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
+        if (T16 == 65536u) run_steps<SH, BLK, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
+        else               run_steps<SH, BLK, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
     } else {
-        net = run_steps<SH, BLK, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
+        run_steps<SH, BLK, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
     }
     // every variant of run_steps ends with a group barrier: the entries are final here
 
     // ---- a7: stage-out (:164): whole packed words of the window ---------------------------------
     for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
         const uint32_t jw = idx / NW, iw = idx - jw * NW;
-        P.lat[(size_t)((wy0 + jw) & LWm) * LW + ((wx0 + iw) & LWm)] = gather_word<SH>(S, iw, jw);
+        const uint32_t word = gather_word<SH>(S, iw, jw);
+        P.lat[(size_t)((wy0 + jw) & LWm) * LW + ((wx0 + iw) & LWm)] = word;
+        net -= x_moment(word, iw);
     }
 
     // counters: net deposits (one atomic per warp) and the tracked height of site (0,0): the site west
