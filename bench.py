@@ -157,6 +157,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="OCT_OPT_KERNEL value: 0 auto, 1 bit-packed, 2 link-entry variant B")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-heights", action="store_true", help="skip timing oct_heights (needs a 4*L*L byte buffer)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -227,6 +228,7 @@ def main():
         tt = torch.tensor([total_ms, sweep_ms], dtype=torch.float64, device=sim.device)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         total_ms, sweep_ms = float(tt[0]), float(tt[1])
+    peaks = measured_peaks()
     attempts_per_step = M * L * L
     value = world * args.steps * attempts_per_step / (total_ms * 1e-3)
 
@@ -236,7 +238,6 @@ def main():
     assert S[2] == h00 and S[3] == net and S[0] + L * L * h00 == L * L // 2 + 2 * net, "inconsistent state"
 
     # ---- roofline of the dominant kernel (sweep): issue-slot bound ---------------------------------
-    peaks = measured_peaks()
     n_sweep_launches = args.steps * M * 4
     launch_s = sweep_ms * 1e-3 / n_sweep_launches
     attempts_per_launch = L * L / 4
@@ -254,6 +255,29 @@ def main():
                 "peak_src": f"148 SM x 4 SMSP x 32 lanes x sm_max_mhz ({peaks['src']})",
                 "hbm_gbs_of_sweep": 0.5 * (1.0 + 4.0 / (1 << args.log2D)) ** 2 * attempts_per_launch / launch_s / 1e9,
                 "sweep_share_of_step": sweep_ms / total_ms}
+
+    # ---- observables (a8/a9): HBM-bound kernels, timed alone, algorithmic bytes / time -------------------
+    def time_call(fn, reps=5):
+        fn(); torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream); torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    lat_bytes = L * L // 4
+    observables = {}
+    for name, fn, nbytes in (("oct_width2", lambda: sim.oct_width2(w2_out), lat_bytes),
+                             ("oct_autocorr", lambda: sim.oct_autocorr(snap, anchor, ac_out), 2 * lat_bytes)):
+        ms = time_call(fn)
+        observables[name] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm": nbytes / ms / 1e6 / peaks["hbm_gbs"]}
+    if L <= (1 << 16) and not args.no_heights:
+        hbuf = torch.empty((L, L), dtype=torch.int32, device=sim.device)
+        ms = time_call(lambda: sim.oct_heights(hbuf), reps=3)
+        nbytes = lat_bytes + 4 * L * L
+        observables["oct_heights"] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm": nbytes / ms / 1e6 / peaks["hbm_gbs"]}
+        del hbuf
 
     # ---- e2e: same step through the C ABI with HOST buffers ------------------------------------------
     e2e = None
@@ -304,7 +328,7 @@ def main():
                 "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16) else None,
                 "dtype": "u32", "data": "synthetic", "config": workload_config(args), "clocks": clocks, "e2e": e2e,
-                "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+                "gpu_launches": launches, "roofline": roofline, "observables": observables, "cpu_baseline": cpu,
                 "paper_context": "PAPER.md:276 ~9e9 attempts/s on Kepler GPUs (other hardware; context, not a target)"}
         print(json.dumps(line), flush=True)
     sim.close()

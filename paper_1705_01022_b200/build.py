@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboct_b200.so")
 SOURCES = ["oct_api.cu"]
-HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "philox.cuh", os.path.join("..", "..", "include", "oct.h")]
+HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "observe_rows.cuh", "philox.cuh", os.path.join("..", "..", "include", "oct.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "--use_fast_math", "-Xptxas", "-v"]
 

@@ -1,0 +1,246 @@
+// Row-streaming kernels for height reconstruction (a8) and the W^2 / C_h reductions (a9), second version.
+//
+// One warp owns one word-row (4 site rows, L/4 packed words).  Per chunk every lane takes RUN
+// *consecutive* words (RUN/4 coalesced 128-bit loads; the warp reads 128*RUN contiguous bytes), walks
+// them in registers and only then the warp does ONE shuffle scan to place the lanes' runs one after the
+// other -- instead of a 64-bit scan per word as in the first version (profiles/r1_a: 554 GB/s).
+//
+// Inside a word the four site rows are handled byte-parallel: byte j of a register belongs to site row
+// 4*wy + j.  With P_i = number of up-links among the first i sites of the row (bytewise prefix sums of
+// the sigma_x bits) the height of site (i, j) of the word is
+//       e_ij = left_j + 2 P_ij - i ,      left_j = height just west of the word in row j.
+// The rows of one word differ by at most a few units (vertical neighbours differ by exactly 1), so
+// left_j = left_0 + d_j with |d_j| <= 5 and the 16 heights are   r0 + H_ij ,   r0 = left_0 - 16 ,
+//       H_i = dq + 2 P_i - i * 0x01010101 ,   dq_j = d_j + 16      (all bytes stay in 7..25),
+// which turns sum e and sum e^2 over the word into  16 r0 + sum H,  16 r0^2 + 2 r0 sum H + sum H^2  with
+// the byte sums done by DP4A.  d_j needs no scan: at the first word of a run it is read off the
+// sigma_y bits of that word's first column, and it advances by 2 (P4_j - P4_0) per word (curl-freeness).
+// Lane sums are kept relative to the unknown height s at the start of the lane's run (32-bit), and
+// widened to int64 once per run:  sum (s + r)^2 = n s^2 + 2 s sum r + sum r^2.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "observe.cuh"
+
+namespace octb {
+
+constexpr uint32_t kOnes = 0x01010101u;
+
+// running state of one lattice stream inside a lane's run
+struct RowRun {
+    int r0;          // left_0 - 16, relative to the height at the start of the run
+    uint32_t dq;     // bytes d_j + 16
+};
+
+// bytewise prefix counts of the sigma_x bits of a word: P[i-1] byte j = #up-links among sites 0..i-1 of row j
+__device__ __forceinline__ void prefix_counts(uint32_t w, uint32_t (&P)[4])
+{
+    P[0] = w & kOnes;
+    P[1] = P[0] + ((w >> 2) & kOnes);
+    P[2] = P[1] + ((w >> 4) & kOnes);
+    P[3] = P[2] + ((w >> 6) & kOnes);
+}
+
+// H_i bytes (heights of the word's sites minus r0) and the advance of the run state to the next word
+__device__ __forceinline__ void word_heights(uint32_t w, RowRun& st, uint32_t (&H)[4], int& r0_here)
+{
+    uint32_t P[4];
+    prefix_counts(w, P);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) H[i] = st.dq - (uint32_t)(i + 1) * kOnes + 2u * P[i];
+    r0_here = st.r0;
+    const uint32_t t0 = P[3] & 0xFFu;
+    st.r0 += 2 * (int)t0 - 4;
+    st.dq = st.dq + 2u * P[3] - 2u * t0 * kOnes;
+}
+
+// d_j + 16 for the heights just west of word w, from the word's own first column:
+//   h(x0-1, j) - h(x0-1, 0) = [sum_{j'=1..j} sigma_y(x0, j')] - [sigma_x(x0, j) - sigma_x(x0, 0)]
+__device__ __forceinline__ uint32_t run_start_dq(uint32_t w)
+{
+    const int x0 = (int)(w & 1u), x1 = (int)((w >> 8) & 1u), x2 = (int)((w >> 16) & 1u), x3 = (int)((w >> 24) & 1u);
+    const int y1 = 2 * (int)((w >> 9) & 1u) - 1, y2 = y1 + 2 * (int)((w >> 17) & 1u) - 1, y3 = y2 + 2 * (int)((w >> 25) & 1u) - 1;
+    const int d1 = y1 - 2 * (x1 - x0), d2 = y2 - 2 * (x2 - x0), d3 = y3 - 2 * (x3 - x0);
+    return 16u | ((uint32_t)(16 + d1) << 8) | ((uint32_t)(16 + d2) << 16) | ((uint32_t)(16 + d3) << 24);
+}
+
+__device__ __forceinline__ int warp_inclusive_scan_i32(int v, int lane)
+{
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const int u = __shfl_up_sync(0xFFFFFFFFu, v, off);
+        if (lane >= off) v += u;
+    }
+    return v;
+}
+
+template <int RUN>
+__device__ __forceinline__ void load_run(const uint32_t* __restrict__ p, uint32_t (&w)[RUN])
+{
+#pragma unroll
+    for (int q = 0; q < RUN / 4; ++q) {
+        const uint4 v = reinterpret_cast<const uint4*>(p)[q];
+        w[4 * q + 0] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
+    }
+}
+
+constexpr int kRows2Warps = 8;
+
+// RUN words per lane per chunk: 16 for L >= 2048 (chunk = 512 words), 4 below (any L >= 16 works:
+// lanes beyond L/16 idle).
+template <int MODE, int RUN>
+__global__ void __launch_bounds__(kRows2Warps * 32) rows2_kernel(const RowsParams P)
+{
+    static_assert(MODE == kModeWidth2 || MODE == kModeAutocorr, "heights are written by heights_kernel");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t LW = P.L >> 2;
+    const uint32_t wy = blockIdx.x * kRows2Warps + warp;     // word-row of this warp
+    long long s1 = 0, s2 = 0, s3 = 0;
+
+    if (wy < LW) {
+        const uint32_t* rowA = P.latA + (size_t)wy * LW;
+        const uint32_t* rowB = MODE == kModeAutocorr ? P.latB + (size_t)wy * LW : nullptr;
+        // height just west of site 0 of site row 4*wy, relative to h(0,0):  h(-1,y) = h(0,y) - sigma_x(0,y)
+        int carryA = P.anchorA[4 * wy] - ((rowA[0] & 1u) ? 1 : -1);
+        int carryB = 0;
+        if constexpr (MODE == kModeAutocorr) carryB = P.anchorB[4 * wy] - ((rowB[0] & 1u) ? 1 : -1);
+        const uint32_t lanes_used = LW / RUN < 32u ? LW / RUN : 32u;
+        const bool on = (uint32_t)lane < lanes_used;
+
+        for (uint32_t wx0 = 0; wx0 < LW; wx0 += 32 * RUN) {
+            const uint32_t wx = wx0 + lane * RUN;
+            uint32_t wa[RUN], wb[RUN];
+            if (on) {
+                load_run<RUN>(rowA + wx, wa);
+                if constexpr (MODE == kModeAutocorr) load_run<RUN>(rowB + wx, wb);
+            } else {
+#pragma unroll
+                for (int k = 0; k < RUN; ++k) { wa[k] = 0x05050505u; wb[k] = 0x05050505u; }   // zero net slope
+            }
+
+            {
+                // heights relative to the (still unknown) height s at the start of this lane's run
+                RowRun a{-16, run_start_dq(wa[0])}, b{-16, 0};
+                if constexpr (MODE == kModeAutocorr) b.dq = run_start_dq(wb[0]);
+                int ra1 = 0, rb1 = 0;            // sum r_A, sum r_B over the run
+                unsigned int q = 0;              // Width2: sum r_A^2; Autocorr: sum r_A r_B  (>= 0 not required: int below)
+                int qx = 0;
+#pragma unroll
+                for (int k = 0; k < RUN; ++k) {
+                    uint32_t HA[4]; int r0a;
+                    word_heights(wa[k], a, HA, r0a);
+                    const int hsa = (int)__dp4a(HA[0] + HA[1] + HA[2] + HA[3], kOnes, 0u);
+                    ra1 += 16 * r0a + hsa;
+                    if constexpr (MODE == kModeWidth2) {
+                        const unsigned int sq = __dp4a(HA[0], HA[0], __dp4a(HA[1], HA[1], __dp4a(HA[2], HA[2], __dp4a(HA[3], HA[3], 0u))));
+                        q += (unsigned int)(16 * r0a * r0a + 2 * r0a * hsa) + sq;
+                    } else {
+                        uint32_t HB[4]; int r0b;
+                        word_heights(wb[k], b, HB, r0b);
+                        const int hsb = (int)__dp4a(HB[0] + HB[1] + HB[2] + HB[3], kOnes, 0u);
+                        rb1 += 16 * r0b + hsb;
+                        const unsigned int cr = __dp4a(HA[0], HB[0], __dp4a(HA[1], HB[1], __dp4a(HA[2], HB[2], __dp4a(HA[3], HB[3], 0u))));
+                        qx += 16 * r0a * r0b + r0a * hsb + r0b * hsa + (int)cr;
+                    }
+                }
+                // place the runs: exclusive scan of the runs' net slope of site row 0
+                const int totA = a.r0 + 16;
+                const int inclA = warp_inclusive_scan_i32(totA, lane);
+                const long long sA = carryA + inclA - totA;
+                carryA += __shfl_sync(0xFFFFFFFFu, inclA, 31);
+                constexpr long long n = 16 * RUN;
+                if constexpr (MODE == kModeWidth2) {
+                    if (on) {
+                        s1 += n * sA + ra1;
+                        s2 += n * sA * sA + 2 * sA * ra1 + (long long)(int)q;
+                    }
+                } else {
+                    const int totB = b.r0 + 16;
+                    const int inclB = warp_inclusive_scan_i32(totB, lane);
+                    const long long sB = carryB + inclB - totB;
+                    carryB += __shfl_sync(0xFFFFFFFFu, inclB, 31);
+                    if (on) {
+                        s1 += n * sA + ra1;
+                        s2 += n * sB + rb1;
+                        s3 += n * sA * sB + sA * rb1 + sB * ra1 + qx;
+                    }
+                }
+            }
+        }
+    }
+
+    if constexpr (MODE != kModeHeights) {
+        __shared__ long long red[3][kRows2Warps];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            s1 += __shfl_xor_sync(0xFFFFFFFFu, s1, off);
+            s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, off);
+            if constexpr (MODE == kModeAutocorr) s3 += __shfl_xor_sync(0xFFFFFFFFu, s3, off);
+        }
+        if (lane == 0) { red[0][warp] = s1; red[1][warp] = s2; red[2][warp] = s3; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            long long t1 = 0, t2 = 0, t3 = 0;
+            for (int w = 0; w < kRows2Warps; ++w) { t1 += red[0][w]; t2 += red[1][w]; t3 += red[2][w]; }
+            atomicAdd(&P.out[0], (unsigned long long)t1);
+            atomicAdd(&P.out[1], (unsigned long long)t2);
+            if constexpr (MODE == kModeAutocorr) atomicAdd(&P.out[2], (unsigned long long)t3);
+            if (blockIdx.x == 0) {
+                if constexpr (MODE == kModeWidth2) {
+                    P.out[2] = P.countersA[1];             // c = h(0,0)
+                    P.out[3] = P.countersA[0];             // net
+                } else {
+                    P.out[3] = P.countersA[1];             // c_t
+                    P.out[4] = (unsigned long long)P.snapB[0];   // c_s
+                }
+            }
+        }
+    }
+}
+
+// Heights (a8): the output (16 bytes per site row per word) dwarfs the input, so the lanes take
+// *adjacent* words -- every store instruction of the warp writes 512 contiguous bytes -- and the warp
+// pays one 32-bit shuffle scan per 32 words (site row 0 only; the other three rows hang off it through
+// dq).  UNR independent word-groups are loaded up front for memory-level parallelism.
+template <int UNR>
+__global__ void __launch_bounds__(kRows2Warps * 32) heights_kernel(const RowsParams P)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t LW = P.L >> 2;
+    const uint32_t wy = blockIdx.x * kRows2Warps + warp;
+    if (wy >= LW) return;
+    const uint32_t* row = P.latA + (size_t)wy * LW;
+    const int h00 = (int)(long long)P.countersA[1];
+    int carry = P.anchorA[4 * wy] - ((row[0] & 1u) ? 1 : -1) + h00;     // h(-1, 4 wy)
+    int* out = P.heights + (size_t)(4 * wy) * P.L;
+
+    for (uint32_t wx0 = 0; wx0 < LW; wx0 += 32 * UNR) {
+        uint32_t w[UNR];
+#pragma unroll
+        for (int k = 0; k < UNR; ++k) {
+            const uint32_t wx = wx0 + 32 * k + lane;
+            w[k] = wx < LW ? row[wx] : 0x05050505u;                     // zero net slope past a short row
+        }
+#pragma unroll
+        for (int k = 0; k < UNR; ++k) {
+            const uint32_t wx = wx0 + 32 * k + lane;
+            const int tot = 2 * __popc(w[k] & 0x55u) - 4;
+            const int incl = warp_inclusive_scan_i32(tot, lane);
+            RowRun st{carry + incl - tot - 16, run_start_dq(w[k])};
+            carry += __shfl_sync(0xFFFFFFFFu, incl, 31);
+            uint32_t H[4]; int r0;
+            word_heights(w[k], st, H, r0);
+            if (wx < LW) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int4 v = make_int4(r0 + (int)((H[0] >> (8 * j)) & 0xFFu), r0 + (int)((H[1] >> (8 * j)) & 0xFFu),
+                                             r0 + (int)((H[2] >> (8 * j)) & 0xFFu), r0 + (int)((H[3] >> (8 * j)) & 0xFFu));
+                    __stcs(reinterpret_cast<int4*>(out + (size_t)j * P.L + 4 * wx), v);   // streaming: never re-read here
+                }
+            }
+        }
+    }
+}
+
+}  // namespace octb

@@ -11,6 +11,7 @@
 
 #include "../../include/oct.h"
 #include "observe.cuh"
+#include "observe_rows.cuh"
 #include "philox.cuh"
 #include "sweep.cuh"
 #include "sweep_links.cuh"
@@ -175,6 +176,15 @@ int ensure_device(oct_ctx* c)
     return OCT_OK;
 }
 
+// one warp per word-row; 16 words per lane per chunk once a row holds at least one full chunk
+template <int MODE>
+void launch_rows(const RowsParams& rp, uint32_t LW, cudaStream_t st)
+{
+    const unsigned blocks = (LW + kRows2Warps - 1) / kRows2Warps;
+    if (LW >= 512u) rows2_kernel<MODE, 16><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
+    else            rows2_kernel<MODE, 4><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
+}
+
 int launch_anchor(oct_ctx* c, const uint32_t* lat, int32_t* anchor, cudaStream_t st)
 {
     column_anchor_kernel<<<1, kAnchorThreads, 0, st>>>(lat, c->L, anchor);
@@ -290,7 +300,7 @@ int oct_heights(oct_ctx* c, int32_t* heights_dev, void* stream)
     RowsParams rp{};
     rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters(); rp.heights = heights_dev; rp.L = c->L;
     const uint32_t LW = c->L >> 2;
-    rows_kernel<kModeHeights><<<(LW + kRowsWarps - 1) / kRowsWarps, kRowsWarps * 32, 0, st>>>(rp);
+    heights_kernel<4><<<(LW + kRows2Warps - 1) / kRows2Warps, kRows2Warps * 32, 0, st>>>(rp);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;
@@ -307,7 +317,7 @@ int oct_width2(oct_ctx* c, int64_t* out_dev, void* stream)
     rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters();
     rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
     const uint32_t LW = c->L >> 2;
-    rows_kernel<kModeWidth2><<<(LW + kRowsWarps - 1) / kRowsWarps, kRowsWarps * 32, 0, st>>>(rp);
+    launch_rows<kModeWidth2>(rp, LW, st);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;
@@ -339,7 +349,7 @@ int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_a
     rp.snapB = reinterpret_cast<const long long*>(snapshot_anchor_dev);
     rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
     const uint32_t LW = c->L >> 2;
-    rows_kernel<kModeAutocorr><<<(LW + kRowsWarps - 1) / kRowsWarps, kRowsWarps * 32, 0, st>>>(rp);
+    launch_rows<kModeAutocorr>(rp, LW, st);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;

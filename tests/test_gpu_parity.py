@@ -153,7 +153,8 @@ def test_flat_shifted_symmetry_on_gpu():
     a.close(); b.close(); orc.close()
 
 
-@pytest.mark.parametrize("L,seed,off", [(16, 1, 0), (64, 2, -7), (128, 5, 3), (256, 3, 1000), (1024, 4, -123456)])
+@pytest.mark.parametrize("L,seed,off", [(16, 1, 0), (32, 9, 2), (64, 2, -7), (128, 5, 3), (256, 3, 1000), (1024, 4, -123456),
+                                        (2048, 6, 77), (4096, 7, -40000)])
 def test_heights_and_sums_on_synthetic_surfaces(L, seed, off):
     """Reconstruction / reduction kernels on surfaces unrelated to the dynamics (rough, ragged L)."""
     h = wl.separable_surface(L, seed, off)
