@@ -1,0 +1,133 @@
+"""GPU parity at BASELINE.json's full sizes (configs 4 and 5: L = 2^16 and 2^17), in the launch
+configuration bench.py times.
+
+The oracle cannot sweep 2^32 sites in seconds, but it does not have to: a domain sweep depends only on
+its own window, so running only the domains that meet a box reproduces the full run inside the box
+shrunk by 4(D+2) sites per MCS (tests/test_oracle_dd.py::test_filtered_run_reproduces_the_interior pins
+that tool against complete runs).  Here the GPU's lattice before and after one MCS is exported, the oracle
+replays that MCS on sampled boxes (one of them across the periodic seam, one around the tracked origin
+site), and the packed words inside the boxes must be identical.  Properties that hold at any size cover
+the rest: slope conservation per row / column, the height-sum identity, C_h(s,s) sums == W^2 sums.
+"""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from paper_1705_01022_b200 import binding, workloads as wl
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def interior_words(x0, y0, w, h, margin, L):
+    """index arrays (wy, wx) of the packed words lying entirely inside the box shrunk by `margin`"""
+    xa, xb = x0 + margin, x0 + w - margin          # site range [xa, xb)
+    ya, yb = y0 + margin, y0 + h - margin
+    wxs = (np.arange((xa + 3) // 4, xb // 4)) % (L // 4)
+    wys = (np.arange((ya + 3) // 4, yb // 4)) % (L // 4)
+    assert len(wxs) > 8 and len(wys) > 8
+    return np.ix_(wys, wxs)
+
+
+_ORACLES = {}
+
+
+def oracle_for(L, seed):
+    """One oracle state per lattice size for the whole module (creating a 2^32-site state takes ~10 s)."""
+    if L not in _ORACLES:
+        _ORACLES[L] = Oracle(L, seed)
+    return _ORACLES[L]
+
+
+def replay_boxes(L, seed, code, log2D, p, q, pre, t, h00, net, post, boxes, h00_after=None):
+    D = 1 << log2D
+    margin = 4 * (D + 2)
+    orc = oracle_for(L, seed)
+    for (x0, y0) in boxes:
+        w = h = 2 * margin + 4 * D
+        orc.set_lattice(pre, h00=h00, net=net, t=t)
+        orc.set_filter(True, x0 % L, y0 % L, w, h)
+        orc.sweep(1, p, q, code)
+        ix = interior_words(x0, y0, w, h, margin, L)
+        got, want = post[ix], orc.lattice[ix]
+        assert (got == want).all(), f"box ({x0},{y0}): {(got != want).sum()} of {got.size} words differ"
+        assert (want != pre[ix]).any(), "the replayed MCS changed nothing inside the box"
+        if h00_after is not None and x0 < 0 and y0 < 0:        # the box around the origin site: its tracked height too
+            assert orc.h00 == h00_after
+    orc.set_filter(False)
+
+
+def popcount_rows(words, mask):
+    """number of set bits under `mask` per word-row and per word-column (uint64 sums)"""
+    v = words & np.uint32(mask)
+    v = v - ((v >> 1) & np.uint32(0x55555555))
+    v = (v & np.uint32(0x33333333)) + ((v >> 2) & np.uint32(0x33333333))
+    v = (v + (v >> 4)) & np.uint32(0x0F0F0F0F)
+    v = (v * np.uint32(0x01010101)) >> 24
+    return v.sum(axis=1, dtype=np.uint64), v.sum(axis=0, dtype=np.uint64)
+
+
+def check_invariants(sim, words):
+    L = sim.L
+    # each site row holds L/2 up-slopes in x, each site column L/2 up-slopes in y (periodic closure);
+    # checked on 1024 sampled word-rows and word-columns
+    pick = np.sort(np.random.default_rng(5).choice(L // 4, size=min(1024, L // 4), replace=False))
+    some_rows, some_cols = words[pick, :], np.ascontiguousarray(words[:, pick])
+    for j in range(4):
+        rows, _ = popcount_rows(some_rows, 0x55 << (8 * j))
+        assert (rows == L // 2).all()
+    for i in range(4):
+        _, cols = popcount_rows(some_cols, 0x02020202 << (2 * i))
+        assert (cols == L // 2).all()
+    S1, S2, c, net = (int(v) for v in sim.oct_width2().cpu().numpy())
+    h00, net2 = sim.oct_counters()
+    assert (c, net) == (h00, net2)
+    assert S1 + L * L * c == L * L // 2 + 2 * net            # sum of heights: flat start + 2 per deposit
+    snap, anchor = sim.oct_snapshot()
+    A = [int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy()]
+    assert A[0] == A[1] == S1 and A[2] == S2 and A[3] == A[4] == c      # C_h(s,s) = W^2(s)
+    del snap
+    return S1, S2, c, net
+
+
+@pytest.mark.parametrize("log2D,kernel", [(6, binding.OCT_KERNEL_AUTO), (7, binding.OCT_KERNEL_AUTO), (8, binding.OCT_KERNEL_AUTO)])
+def test_config3_L65536_sampled_boxes(log2D, kernel):
+    """BASELINE config 4: L = 2^16, p = 1, q = 0, flat start, seed 1, DTrDB TC=1,1."""
+    L, seed, p, q = 1 << 16, 1, 1.0, 0.0
+    code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, log2D)
+    sim = binding.Sim(L, seed)
+    sim.oct_set_option(binding.OCT_OPT_KERNEL, kernel)
+    # the very first MCS, from the flat state (acceptance 1/2)
+    pre = sim.oct_export()
+    assert (pre == 0x33CC33CC).all()
+    sim.oct_sweep(1, p, q, code)
+    post = sim.oct_export()
+    replay_boxes(L, seed, code, log2D, p, q, pre, 0, 0, 0, post, [(1000, 2000), (L - 700, L - 900)])
+    # an evolved state (what bench.py times): MCS 24 -> 25
+    sim.oct_sweep(23, p, q, code)
+    sim.oct_export(pre)
+    h00, net = sim.oct_counters()
+    sim.oct_sweep(1, p, q, code)
+    sim.oct_export(post)
+    D = 1 << log2D
+    margin = 4 * (D + 2)
+    replay_boxes(L, seed, code, log2D, p, q, pre, 24, h00, net, post,
+                 [(31337, 4242), (L - 5 * D, 17 * D + 3), (-margin - 2 * D, -margin - 2 * D)], h00_after=sim.oct_counters()[0])
+    S1, S2, c, net = check_invariants(sim, post)
+    assert net > 0 and S2 > 0
+    sim.close()
+
+
+def test_config4_L131072_sampled_boxes():
+    """BASELINE config 5: L = 2^17 (4 GiB packed), same scheme: evolved-state MCS replayed on boxes."""
+    L, seed, p, q, log2D = 1 << 17, 1, 1.0, 0.0, 6
+    code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, log2D)
+    sim = binding.Sim(L, seed)
+    sim.oct_sweep(6, p, q, code)
+    pre = sim.oct_export()
+    h00, net = sim.oct_counters()
+    sim.oct_sweep(1, p, q, code)
+    post = sim.oct_export()
+    replay_boxes(L, seed, code, log2D, p, q, pre, 6, h00, net, post, [(99991, 70001), (L - 300, L - 400)])
+    check_invariants(sim, post)
+    sim.close()
