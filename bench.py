@@ -170,7 +170,7 @@ def main():
         return
 
     import torch
-    from paper_1705_01022_b200 import binding, workloads as wl
+    from paper_1705_01022_b200 import binding, replicas, workloads as wl
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product has no CPU path (use --impl reference for the oracle)")
@@ -182,7 +182,7 @@ def main():
 
     L, M = args.L, args.mcs_per_step
     code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, args.log2D)
-    seed = wl.rank_seed(args.seed, rank)
+    seed = replicas.replica_seed(args.seed, rank)
     sim = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
     sim.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)
     stream = torch.cuda.current_stream()
@@ -224,13 +224,10 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     total_ms = e0.elapsed_time(e1)
     sweep_ms = sum(a.elapsed_time(b) for a, b in evs)
-    if dist is not None:
-        tt = torch.tensor([total_ms, sweep_ms], dtype=torch.float64, device=sim.device)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms, sweep_ms = float(tt[0]), float(tt[1])
+    total_ms, sweep_ms = replicas.max_over_ranks([total_ms, sweep_ms], dist, sim.device)
     peaks = measured_peaks()
     attempts_per_step = M * L * L
-    value = world * args.steps * attempts_per_step / (total_ms * 1e-3)
+    value = replicas.aggregate_throughput(attempts_per_step, args.steps, world, total_ms)
 
     # sanity of the state that was timed: sums are consistent with the counters
     S = [int(v) for v in w2_out.cpu().numpy()]
@@ -308,11 +305,8 @@ def main():
         ms = e0.elapsed_time(e1)
         wall = (time.perf_counter() - t0) * 1e3
         ms = max(ms, wall)
-        if dist is not None:
-            tt = torch.tensor([ms], dtype=torch.float64, device=sim.device)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ms = float(tt[0])
-        e2e = {"value": world * ke * attempts_per_step / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nb,
+        ms = replicas.max_over_ranks([ms], dist, sim.device)[0]
+        e2e = {"value": replicas.aggregate_throughput(attempts_per_step, ke, world, ms), "unit": UNIT, "h2d_bytes_per_step": nb,
                "d2h_bytes_per_step": nb + 72, "steps": ke, "ms_per_step": ms / ke}
 
     # ---- the oracle timed on this box's host cores (rank 0, N = 1 only) -------------------------------
