@@ -81,6 +81,7 @@ def lib():
         L.orc_heights_rowpath.argtypes = [vp, vp]; L.orc_heights_rowpath.restype = None
         L.orc_sums.argtypes = [vp, vp]; L.orc_sums.restype = i32
         L.orc_autocorr_sums.argtypes = [vp, vp, vp]; L.orc_autocorr_sums.restype = i32
+        L.orc_slope_autocorr_sums.argtypes = [vp, vp, vp]; L.orc_slope_autocorr_sums.restype = i32
         _lib = L
     return _lib
 
@@ -242,6 +243,20 @@ class Oracle:
         if rc:
             raise RuntimeError(f"orc_autocorr_sums -> {rc}")
         return tuple(int(v) for v in o)
+
+    def slope_autocorr_sums(self, snap: "Oracle"):
+        """(sum nx_t nx_s, sum ny_t ny_s, sum nx_t, sum ny_t, sum nx_s, sum ny_s) against a snapshot."""
+        o = np.zeros(6, dtype=np.int64)
+        rc = self._l.orc_slope_autocorr_sums(self._h, snap._h, o.ctypes.data)
+        if rc:
+            raise RuntimeError(f"orc_slope_autocorr_sums -> {rc}")
+        return tuple(int(v) for v in o)
+
+    def c_s(self, snap: "Oracle") -> Fraction:
+        """C_s(t,s) over all 2 L^2 slope variables, exact."""
+        xx, yy, xt, yt, xs, ys = self.slope_autocorr_sums(snap)
+        M = 2 * self.L * self.L
+        return Fraction(M * (xx + yy) - (xt + yt) * (xs + ys), M * M)
 
     def c_h(self, snap: "Oracle") -> Fraction:
         St, Ss, Sts, _, _ = self.autocorr_sums(snap)

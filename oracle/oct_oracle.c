@@ -13,13 +13,15 @@
  *                      DT, DTr         Sec. 3.0.2 :142-146, Sec. 3.0.3 :148-150          -> orc_sweep_dd
  *   - block-layer single-hit DB / DT   Sec. 3.1 :168-174                                 -> domain_sweep
  *   - roughness W^2, autocorr C_h      Eq. (3) :61, Eq. (6) :92-98                       -> orc_sums, orc_autocorr_sums
+ *   - slope (lattice-gas) autocorr C_s :85-88 (unnumbered equation before Eq. (6))       -> orc_slope_autocorr_sums
  *   - RNG (paper silent)               Philox4x32-10, Salmon et al. SC'11; keying = DESIGN.md R19
  *
  * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): Philox known-answer vectors and cuRAND's host
  * implementation; flat-state constants; brute-force of the height definition on the 4x4 lattice;
  * row/column conservation and curl-freeness; tracked vs recomputed heights (two paths); order
  * independence of every DD phase; complement symmetry; split invariance; attempt-trace properties
- * (coverage, uniformity, cell geometry); W^2(0)=1/4; C_h(s,s)=W^2(s); KPZ growth exponent band.
+ * (coverage, uniformity, cell geometry); W^2(0)=1/4; C_h(s,s)=W^2(s); C_s(s,s)=1/4, C_s against the
+ * complement = -1/4 and against slopes taken straight from a height array; KPZ growth exponent band.
  * Absolute W^2(t)/C(t,s) curves of the paper are figures only: "parity unpinned" against those.
  *
  * Conventions.  Site (x,y), 0 <= x,y < L, periodic.  sigma_x(x,y) = h(x,y)-h(x-1,y),
@@ -511,6 +513,24 @@ int orc_autocorr_sums(const orc_state *now, const orc_state *snap, int64_t out[5
     }
     free(ht); free(hs);
     out[0] = St; out[1] = Ss; out[2] = Sts; out[3] = ct; out[4] = cs;
+    return 0;
+}
+
+/* Slope autocorrelation (:85-88): C_s(t,s) = <n(t,r) n(s,r)> - <n(t)><n(s)> with n the lattice-gas
+ * occupation = the slope bit (:50 "up/down slopes ... particles/holes").  Integer sums, x and y slopes
+ * kept apart: out = {sum nx_t nx_s, sum ny_t ny_s, sum nx_t, sum ny_t, sum nx_s, sum ny_s}. */
+int orc_slope_autocorr_sums(const orc_state *now, const orc_state *snap, int64_t out[6])
+{
+    if (now->L != snap->L) return -1;
+    const uint32_t L = now->L;
+    for (int k = 0; k < 6; ++k) out[k] = 0;
+    for (uint32_t y = 0; y < L; ++y)
+        for (uint32_t x = 0; x < L; ++x) {
+            const int xt = get_sx(now, x, y), yt = get_sy(now, x, y);
+            const int xs = get_sx(snap, x, y), ys = get_sy(snap, x, y);
+            out[0] += xt * xs; out[1] += yt * ys;
+            out[2] += xt; out[3] += yt; out[4] += xs; out[5] += ys;
+        }
     return 0;
 }
 

@@ -82,3 +82,37 @@ def test_kpz_growth_exponent_band_and_rs_agreement():
     # same kinetics up to a prefactor that is not larger for the finer decomposition (:254)
     ratio = dd / rs
     assert (np.abs(ratio - 1) < 0.06).all(), ratio
+
+
+def test_slope_autocorrelation_pins():
+    """C_s of PAPER.md:85-88 on the lattice-gas variables n = slope bit.  Pins that do not go through the
+    oracle's own packing: slopes taken straight from height arrays; the equal-time value 1/4 (n^2 = n,
+    <n> = 1/2 by the periodic closure); the complement -1/4; the flat state against its one-site shift."""
+    from paper_1705_01022_b200.workloads import separable_surface, pack_heights   # seeded input generator, no method arithmetic
+    L = 64
+    ha, hb = separable_surface(L, 11, 5), separable_surface(L, 12, -3)
+    a, b = Oracle(L, 0), Oracle(L, 0)
+    a.set_lattice(pack_heights(ha)); b.set_lattice(pack_heights(hb))
+    nxa, nya = (ha - np.roll(ha, 1, axis=1)) == 1, (ha - np.roll(ha, 1, axis=0)) == 1
+    nxb, nyb = (hb - np.roll(hb, 1, axis=1)) == 1, (hb - np.roll(hb, 1, axis=0)) == 1
+    want = (int((nxa & nxb).sum()), int((nya & nyb).sum()), int(nxa.sum()), int(nya.sum()), int(nxb.sum()), int(nyb.sum()))
+    assert a.slope_autocorr_sums(b) == want
+    N = L * L
+    assert want[2:] == (N // 2,) * 4                                   # half of the slopes point up, always
+    M = 2 * N
+    assert a.c_s(b) == Fraction(M * (want[0] + want[1]) - (want[2] + want[3]) * (want[4] + want[5]), M * M)
+    assert a.c_s(a) == Fraction(1, 4) and b.c_s(b) == Fraction(1, 4)
+    # complement (the surface turned upside down): n -> 1 - n, so <n n'> = 0 and C_s = -1/4
+    c = Oracle(L, 0); c.set_lattice(~pack_heights(ha))
+    assert a.c_s(c) == Fraction(-1, 4)
+    # flat state vs flat shifted (init 1 is its complement, tests/test_oracle_rule.py)
+    f0, f1 = Oracle(L, 0, init=0), Oracle(L, 0, init=1)
+    assert f0.c_s(f0) == Fraction(1, 4) and f0.c_s(f1) == Fraction(-1, 4)
+    # and it decays under the dynamics, from 1/4 at t = s
+    o = Oracle(L, 5); code = scheme(DEV_DTR, BLK_DB, 4)
+    o.sweep(5, 1.0, 0.0, code); s = o.clone()
+    assert o.c_s(s) == Fraction(1, 4)
+    o.sweep(10, 1.0, 0.0, code)
+    assert 0 < o.c_s(s) < Fraction(1, 4)
+    for x in (a, b, c, f0, f1, o, s):
+        x.close()
