@@ -190,6 +190,7 @@ def main():
     snap, anchor = sim.oct_snapshot()
     w2_out = torch.empty(4, dtype=torch.int64, device=sim.device)
     ac_out = torch.empty(5, dtype=torch.int64, device=sim.device)
+    cs_out = torch.empty(6, dtype=torch.int64, device=sim.device)
 
     def step(ev=None):
         if ev:
@@ -266,7 +267,8 @@ def main():
     lat_bytes = L * L // 4
     observables = {}
     for name, fn, nbytes in (("oct_width2", lambda: sim.oct_width2(w2_out), lat_bytes),
-                             ("oct_autocorr", lambda: sim.oct_autocorr(snap, anchor, ac_out), 2 * lat_bytes)):
+                             ("oct_autocorr", lambda: sim.oct_autocorr(snap, anchor, ac_out), 2 * lat_bytes),
+                             ("oct_slope_autocorr", lambda: sim.oct_slope_autocorr(snap, cs_out), 2 * lat_bytes)):
         ms = time_call(fn)
         observables[name] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm": nbytes / ms / 1e6 / peaks["hbm_gbs"]}
     if L <= (1 << 16) and not args.no_heights:

@@ -112,6 +112,13 @@ int oct_snapshot(oct_ctx*, void* lattice_copy_dev, int64_t* anchor_out_dev, void
 int oct_autocorr(oct_ctx*, const void* snapshot_dev, const int64_t* snapshot_anchor_dev,
                  int64_t* out_dev, void* stream);
 
+/* Integer sums for the slope (lattice-gas) autocorrelation C_s(t,s) of PAPER.md:85-88 between the current
+ * lattice and a snapshot (oct_snapshot's lattice copy, 16-byte aligned), n = slope bit:
+ * out_dev[6] = {sum nx_t nx_s, sum ny_t ny_s, sum nx_t, sum ny_t, sum nx_s, sum ny_s} (x and y slopes apart;
+ * the four single sums are L*L/2 for any valid surface).  C_s = oct_cs_from_sums over M = 2 L^2 variables
+ * (or M = L^2 for one direction); C_s(s,s) = 1/4. */
+int oct_slope_autocorr(oct_ctx*, const void* snapshot_dev, int64_t* out_dev, void* stream);
+
 /* Copy the packed lattice device -> host (canonical words).  SYNCHRONISES `stream`. */
 int oct_export(oct_ctx*, void* lattice_host, void* stream);
 /* Copy a packed lattice host -> device (enqueued; the host buffer must stay valid until the stream
@@ -140,6 +147,7 @@ int oct_launch_count(const oct_ctx*, uint64_t* n_out);
 /* Pure host helpers (no device work). */
 double oct_w2_from_sums(uint32_t L, int64_t S1, int64_t S2);                    /* (N*S2 - S1^2)/N^2  */
 double oct_c_from_sums(uint32_t L, int64_t St, int64_t Ss, int64_t Sts);        /* (N*Sts - St*Ss)/N^2 */
+double oct_cs_from_sums(uint64_t M, int64_t n11, int64_t n1t, int64_t n1s);     /* (M*n11 - n1t*n1s)/M^2 */
 double oct_time_per_sweep(uint32_t L, int scheme);   /* 1 for DT/DTr; (1 - N_border/N) for DB/cDB (R9) */
 int    oct_scheme_supported(uint32_t L, int scheme); /* OCT_OK or OCT_EINVAL, same checks as oct_sweep */
 

@@ -21,7 +21,7 @@ EXPORTS = (
     "oct_lattice_bytes", "oct_workspace_bytes", "oct_create", "oct_set_state", "oct_sweep", "oct_heights",
     "oct_width2", "oct_snapshot", "oct_autocorr", "oct_export", "oct_upload", "oct_counters", "oct_mcs",
     "oct_destroy", "oct_strerror", "oct_last_error", "oct_launch_count", "oct_w2_from_sums", "oct_c_from_sums",
-    "oct_time_per_sweep", "oct_scheme_supported", "oct_set_option",
+    "oct_time_per_sweep", "oct_scheme_supported", "oct_set_option", "oct_slope_autocorr", "oct_cs_from_sums",
 )
 OCT_OPT_KERNEL = 1
 OCT_KERNEL_AUTO, OCT_KERNEL_BITPACKED, OCT_KERNEL_LINKS_B = 0, 1, 2
@@ -65,6 +65,7 @@ def load(rebuild_if_stale: bool = True):
         "oct_w2_from_sums": (dbl, [u32, i64, i64]), "oct_c_from_sums": (dbl, [u32, i64, i64, i64]),
         "oct_time_per_sweep": (dbl, [u32, i32]), "oct_scheme_supported": (i32, [u32, i32]),
         "oct_set_option": (i32, [vp, i32, i32]),
+        "oct_slope_autocorr": (i32, [vp, vp, vp, vp]), "oct_cs_from_sums": (dbl, [u64, i64, i64, i64]),
     }
     for name in EXPORTS:
         fn = getattr(L, name)          # AttributeError if a declared symbol is not exported
@@ -99,6 +100,10 @@ def oct_w2_from_sums(L: int, S1: int, S2: int) -> float:
 
 def oct_c_from_sums(L: int, St: int, Ss: int, Sts: int) -> float:
     return float(load().oct_c_from_sums(L, St, Ss, Sts))
+
+
+def oct_cs_from_sums(M: int, n11: int, n1t: int, n1s: int) -> float:
+    return float(load().oct_cs_from_sums(M, n11, n1t, n1s))
 
 
 def oct_time_per_sweep(L: int, scheme: int) -> float:
@@ -191,6 +196,14 @@ class Sim:
             out = self.torch.empty(5, dtype=self.torch.int64, device=self.device)
         self._check(self._l.oct_autocorr(self._h, snapshot.data_ptr(), anchor.data_ptr(), out.data_ptr(),
                                          _stream_ptr(stream)), "oct_autocorr")
+        return out
+
+    def oct_slope_autocorr(self, snapshot, out=None, stream=None):
+        """Device tensor int64[6] = {sum nx_t nx_s, sum ny_t ny_s, sum nx_t, sum ny_t, sum nx_s, sum ny_s}."""
+        if out is None:
+            out = self.torch.empty(6, dtype=self.torch.int64, device=self.device)
+        self._check(self._l.oct_slope_autocorr(self._h, snapshot.data_ptr(), out.data_ptr(), _stream_ptr(stream)),
+                    "oct_slope_autocorr")
         return out
 
     def oct_export(self, host=None, stream=None) -> np.ndarray:

@@ -67,6 +67,42 @@ struct RowsParams {
     uint32_t L;
 };
 
+// ---- slope (lattice-gas) autocorrelation C_s(t,s), PAPER.md:85-88 --------------------------------------
+// n = slope bit.  out = {sum nx_t nx_s, sum ny_t ny_s, sum nx_t, sum ny_t, sum nx_s, sum ny_s}: one streaming
+// pass over both packed lattices (0.5 B/site), six POPC per word pair, grid-stride, int64 atomics per CTA.
+constexpr int kSlopeThreads = 256;
+
+__global__ void __launch_bounds__(kSlopeThreads)
+slope_autocorr_kernel(const uint4* __restrict__ A, const uint4* __restrict__ B, size_t n_vec, unsigned long long* __restrict__ out)
+{
+    constexpr uint32_t MX = 0x55555555u, MY = 0xAAAAAAAAu;
+    unsigned int c[6] = {0, 0, 0, 0, 0, 0};      // per thread: < 2^32 bits even at L = 2^17 with >= 2^10 threads
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec; i += (size_t)gridDim.x * blockDim.x) {
+        const uint4 a = A[i], b = B[i];
+        const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t ab = aw[k] & bw[k];
+            c[0] += __popc(ab & MX); c[1] += __popc(ab & MY);
+            c[2] += __popc(aw[k] & MX); c[3] += __popc(aw[k] & MY);
+            c[4] += __popc(bw[k] & MX); c[5] += __popc(bw[k] & MY);
+        }
+    }
+    __shared__ unsigned long long red[6][kSlopeThreads / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const unsigned int v = __reduce_add_sync(0xFFFFFFFFu, c[k]);      // a warp's total stays far below 2^32
+        if (lane == 0) red[k][warp] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        unsigned long long t = 0;
+        for (int w = 0; w < kSlopeThreads / 32; ++w) t += red[threadIdx.x][w];
+        atomicAdd(&out[threadIdx.x], t);
+    }
+}
+
 // ---- init ------------------------------------------------------------------------------------------
 __global__ void fill_words_kernel(uint4* __restrict__ lat, size_t n_vec, uint32_t word)
 {

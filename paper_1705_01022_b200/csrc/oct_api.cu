@@ -355,6 +355,21 @@ int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_a
     return OCT_OK;
 }
 
+int oct_slope_autocorr(oct_ctx* c, const void* snapshot_dev, int64_t* out_dev, void* stream)
+{
+    if (!c || !snapshot_dev || !out_dev || (reinterpret_cast<uintptr_t>(snapshot_dev) & 15u)) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 6 * sizeof(int64_t), st));
+    const size_t n_vec = (size_t)c->L * c->L / 4 / 16;
+    const size_t want = (n_vec + kSlopeThreads - 1) / kSlopeThreads;
+    const unsigned blocks = (unsigned)(want < 148 * 16 ? want : 148 * 16);
+    slope_autocorr_kernel<<<blocks, kSlopeThreads, 0, st>>>(reinterpret_cast<const uint4*>(c->lat), static_cast<const uint4*>(snapshot_dev),
+                                                           n_vec, reinterpret_cast<unsigned long long*>(out_dev));
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
 int oct_export(oct_ctx* c, void* lattice_host, void* stream)
 {
     if (!c || !lattice_host) return OCT_EINVAL;
@@ -431,6 +446,14 @@ double oct_c_from_sums(uint32_t L, int64_t St, int64_t Ss, int64_t Sts)
     const __int128 N = (__int128)L * L;
     const __int128 num = N * (__int128)Sts - (__int128)St * (__int128)Ss;
     return (double)((long double)num / ((long double)N * (long double)N));
+}
+
+double oct_cs_from_sums(uint64_t M, int64_t n11, int64_t n1t, int64_t n1s)
+{
+    if (M == 0) return 0.0;
+    const __int128 m = (__int128)M;
+    const __int128 num = m * (__int128)n11 - (__int128)n1t * (__int128)n1s;
+    return (double)((long double)num / ((long double)m * (long double)m));
 }
 
 double oct_time_per_sweep(uint32_t L, int scheme)

@@ -171,6 +171,13 @@ def test_heights_and_sums_on_synthetic_surfaces(L, seed, off):
     got = tuple(int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy())
     orc2 = Oracle(L, 0); orc2.set_lattice(wl.pack_heights(h2), h00=off - 5, net=3)
     assert got == orc.autocorr_sums(orc2)
+    # slope autocorrelation against the same second surface, and C_s(s,s) = 1/4
+    cs = tuple(int(v) for v in sim.oct_slope_autocorr(snap).cpu().numpy())
+    assert cs == orc.slope_autocorr_sums(orc2)
+    own = tuple(int(v) for v in sim.oct_slope_autocorr(sim.lattice).cpu().numpy())
+    assert own == (L * L // 2,) * 6
+    assert binding.oct_cs_from_sums(2 * L * L, own[0] + own[1], own[2] + own[3], own[4] + own[5]) == 0.25
+    assert binding.oct_cs_from_sums(2 * L * L, cs[0] + cs[1], cs[2] + cs[3], cs[4] + cs[5]) == pytest.approx(float(orc.c_s(orc2)), rel=1e-12, abs=1e-15)
     sim.close(); orc.close(); orc2.close()
 
 
@@ -188,6 +195,7 @@ def test_aging_snapshot_and_autocorrelation():
         orc.sweep(n, 1.0, 0.0, code); sim.oct_sweep(n, 1.0, 0.0, code)
         A = tuple(int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy())
         assert A == orc.autocorr_sums(osnap)
+        assert tuple(int(v) for v in sim.oct_slope_autocorr(snap).cpu().numpy()) == orc.slope_autocorr_sums(osnap)
         assert binding.oct_c_from_sums(L, A[0], A[1], A[2]) == pytest.approx(float(orc.c_h(osnap)), rel=1e-13)
     sim.close(); orc.close(); osnap.close()
 
