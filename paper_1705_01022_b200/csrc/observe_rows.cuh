@@ -9,14 +9,14 @@
 // 4*wy + j.  With P_i = number of up-links among the first i sites of the row (bytewise prefix sums of
 // the sigma_x bits) the height of site (i, j) of the word is
 //       e_ij = left_j + 2 P_ij - i ,      left_j = height just west of the word in row j.
-// The rows of one word differ by at most a few units (vertical neighbours differ by exactly 1), so
-// left_j = left_0 + d_j with |d_j| <= 5 and the 16 heights are   r0 + H_ij ,   r0 = left_0 - 16 ,
-//       H_i = dq + 2 P_i - i * 0x01010101 ,   dq_j = d_j + 16      (all bytes stay in 7..25),
-// which turns sum e and sum e^2 over the word into  16 r0 + sum H,  16 r0^2 + 2 r0 sum H + sum H^2  with
-// the byte sums done by DP4A.  d_j needs no scan: at the first word of a run it is read off the
-// sigma_y bits of that word's first column, and it advances by 2 (P4_j - P4_0) per word (curl-freeness).
-// Lane sums are kept relative to the unknown height s at the start of the lane's run (32-bit), and
-// widened to int64 once per run:  sum (s + r)^2 = n s^2 + 2 s sum r + sum r^2.
+// Reductions: over a lane's run of <= 64 sites every height stays within +-73 of the height s at the start
+// of the run (rows of one word differ by at most 5 there), so the heights are carried ENTIRELY in unsigned
+// bytes,  H_i = base + 2 P_i - i * 0x01010101  with  base_j = left_j - s + 128,  and sum H, sum H^2 (or
+// sum H_A H_B) are plain DP4A accumulations; the bias and s come off once per run in int64:
+//       sum (s + r)^2 = n s^2 + 2 s sum r + sum r^2 .
+// base needs no scan: at the first word of a run its row differences are read off the sigma_y bits of
+// that word's first column (curl-freeness), and it advances by 2 P_4 - 4 per word.
+// Heights: the same bytes relative to a 32-bit running height r0 (RowRun / word_heights below).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -120,32 +120,41 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows2_kernel(const RowsParam
             }
 
             {
-                // heights relative to the (still unknown) height s at the start of this lane's run
-                RowRun a{-16, run_start_dq(wa[0])}, b{-16, 0};
-                if constexpr (MODE == kModeAutocorr) b.dq = run_start_dq(wb[0]);
-                int ra1 = 0, rb1 = 0;            // sum r_A, sum r_B over the run
-                unsigned int q = 0;              // Width2: sum r_A^2; Autocorr: sum r_A r_B  (>= 0 not required: int below)
-                int qx = 0;
+                // heights relative to the (still unknown) height s at the start of this lane's run, kept ENTIRELY
+                // in bytes: over a run of <= 64 sites they stay within +-73 of s, so H = e - s + 128 is an
+                // unsigned byte and the run's sums are plain DP4A accumulations; the bias comes off once per run
+                uint32_t ba = run_start_dq(wa[0]) + 112u * kOnes, bb = 0;      // bytes left_j - s + 128
+                if constexpr (MODE == kModeAutocorr) bb = run_start_dq(wb[0]) + 112u * kOnes;
+                unsigned int a1 = 0, b1 = 0, qq = 0;     // sum H_A, sum H_B, sum H_A^2 (Width2) or sum H_A H_B (Autocorr)
 #pragma unroll
                 for (int k = 0; k < RUN; ++k) {
-                    uint32_t HA[4]; int r0a;
-                    word_heights(wa[k], a, HA, r0a);
-                    const int hsa = (int)__dp4a(HA[0] + HA[1] + HA[2] + HA[3], kOnes, 0u);
-                    ra1 += 16 * r0a + hsa;
+                    uint32_t PA[4], HA[4];
+                    prefix_counts(wa[k], PA);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) { HA[i] = ba - (uint32_t)(i + 1) * kOnes + 2u * PA[i]; a1 = __dp4a(HA[i], kOnes, a1); }
+                    ba = ba + 2u * PA[3] - 4u * kOnes;
                     if constexpr (MODE == kModeWidth2) {
-                        const unsigned int sq = __dp4a(HA[0], HA[0], __dp4a(HA[1], HA[1], __dp4a(HA[2], HA[2], __dp4a(HA[3], HA[3], 0u))));
-                        q += (unsigned int)(16 * r0a * r0a + 2 * r0a * hsa) + sq;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) qq = __dp4a(HA[i], HA[i], qq);
                     } else {
-                        uint32_t HB[4]; int r0b;
-                        word_heights(wb[k], b, HB, r0b);
-                        const int hsb = (int)__dp4a(HB[0] + HB[1] + HB[2] + HB[3], kOnes, 0u);
-                        rb1 += 16 * r0b + hsb;
-                        const unsigned int cr = __dp4a(HA[0], HB[0], __dp4a(HA[1], HB[1], __dp4a(HA[2], HB[2], __dp4a(HA[3], HB[3], 0u))));
-                        qx += 16 * r0a * r0b + r0a * hsb + r0b * hsa + (int)cr;
+                        uint32_t PB[4], HB[4];
+                        prefix_counts(wb[k], PB);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            HB[i] = bb - (uint32_t)(i + 1) * kOnes + 2u * PB[i];
+                            b1 = __dp4a(HB[i], kOnes, b1);
+                            qq = __dp4a(HA[i], HB[i], qq);
+                        }
+                        bb = bb + 2u * PB[3] - 4u * kOnes;
                     }
                 }
+                constexpr int nn = 16 * RUN;
+                const int ra1 = (int)a1 - 128 * nn;                                   // sum (e_A - s_A)
+                const int rb1 = (int)b1 - 128 * nn;
+                // Width2: sum (H-128)^2 ; Autocorr: sum (H_A-128)(H_B-128)
+                const int q = MODE == kModeWidth2 ? (int)(qq - 256u * a1) + 16384 * nn : (int)(qq - 128u * (a1 + b1)) + 16384 * nn;
+                const int totA = (int)(ba & 0xFFu) - 128, totB = (int)(bb & 0xFFu) - 128;   // net slope of site row 0 over the run
                 // place the runs: exclusive scan of the runs' net slope of site row 0
-                const int totA = a.r0 + 16;
                 const int inclA = warp_inclusive_scan_i32(totA, lane);
                 const long long sA = carryA + inclA - totA;
                 carryA += __shfl_sync(0xFFFFFFFFu, inclA, 31);
@@ -153,17 +162,16 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows2_kernel(const RowsParam
                 if constexpr (MODE == kModeWidth2) {
                     if (on) {
                         s1 += n * sA + ra1;
-                        s2 += n * sA * sA + 2 * sA * ra1 + (long long)(int)q;
+                        s2 += n * sA * sA + 2 * sA * ra1 + q;
                     }
                 } else {
-                    const int totB = b.r0 + 16;
                     const int inclB = warp_inclusive_scan_i32(totB, lane);
                     const long long sB = carryB + inclB - totB;
                     carryB += __shfl_sync(0xFFFFFFFFu, inclB, 31);
                     if (on) {
                         s1 += n * sA + ra1;
                         s2 += n * sB + rb1;
-                        s3 += n * sA * sB + sA * rb1 + sB * ra1 + qx;
+                        s3 += n * sA * sB + sA * rb1 + sB * ra1 + q;
                     }
                 }
             }
