@@ -135,8 +135,9 @@ def run_reference(args, rank: int, world: int):
 
 
 def workload_config(args):
-    return {"workload": f"c3_L{args.L}: octahedron model, L={args.L} periodic, flat start, p=1 q=0, DTrDB TC=1,1 D={1 << args.log2D}",
-            "L": args.L, "p": 1.0, "q": 0.0, "scheme": f"DTrDB,TC=1,1,D={1 << args.log2D}", "mcs_per_step": args.mcs_per_step,
+    name = "DTrDT" if getattr(args, "blk", 0) == 2 else "DTrDB"
+    return {"workload": f"c3_L{args.L}: octahedron model, L={args.L} periodic, flat start, p=1 q=0, {name} TC=1,1 D={1 << args.log2D}",
+            "L": args.L, "p": 1.0, "q": 0.0, "scheme": f"{name},TC=1,1,D={1 << args.log2D}", "mcs_per_step": args.mcs_per_step,
             "burn_in_mcs": args.burn_in, "l2": "inputs larger than L2 (lattice %d MiB)" % (args.L * args.L // 4 >> 20),
             "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
 
@@ -154,6 +155,7 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--ref-L", type=int, default=4096, help="lattice edge of the oracle's timed sample")
     ap.add_argument("--ref-mcs", type=int, default=32)
+    ap.add_argument("--blk", type=int, default=0, help="block layer: 0 DB (the benched DTrDB), 2 DT (DTrDT, PAPER.md:268)")
     ap.add_argument("--kernel", type=int, default=0, help="OCT_OPT_KERNEL value: 0 auto, 1 bit-packed, 2 link-entry variant B")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -181,7 +183,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     L, M = args.L, args.mcs_per_step
-    code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, args.log2D)
+    code = wl.scheme_code(wl.DEV_DTR, args.blk, args.log2D)
     seed = replicas.replica_seed(args.seed, rank)
     sim = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
     sim.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)

@@ -1,0 +1,23 @@
+"""Host-side helpers of the run driver (time grid, effective exponents of Eq. (8))."""
+import math
+
+import pytest
+
+from paper_1705_01022_b200 import run
+
+
+def test_log_grid_is_sorted_unique_and_ends_at_t_max():
+    g = run.log_grid(10_000, 8)
+    assert g[0] == 1 and g[-1] == 10_000 and g == sorted(set(g))
+    assert all(b > a for a, b in zip(g, g[1:]))
+    assert 30 <= len(g) <= 40                                  # ~8 points per decade over 4 decades
+    assert run.log_grid(1, 8) == [1]
+
+
+def test_effective_exponent_recovers_a_power_law():
+    # E = 3 t^0.4828 (2 beta with beta = 0.2414) -> e_eff = 0.4828 between any two points
+    f = lambda t: 3.0 * t ** 0.4828
+    for t0, t1 in ((10, 20), (100, 1000), (7, 5000)):
+        assert run.eff_exponent(f(t1), t1, f(t0), t0) == pytest.approx(0.4828, rel=1e-12)
+    assert run.eff_exponent(1.0, 10, 0.0, 5) is None and run.eff_exponent(1.0, 5, 1.0, 5) is None
+    assert math.isclose(run.eff_exponent(0.5, 4, 1.0, 2), -1.0)
