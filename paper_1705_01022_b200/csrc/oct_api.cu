@@ -67,10 +67,13 @@ struct SweepLaunch {
     int threads, smem, dpb;
 };
 
+#ifndef OCT_CELLS_PER_WARP
+#define OCT_CELLS_PER_WARP 128   // bit-packed kernel: cells carried by one warp (4 per lane; 8 overflows the instruction cache, profiles/r1_a)
+#endif
 constexpr int pick_wpd(int log2d, int tcx, int tcy)
 {
     const int ncell = ((1 << log2d) / (4 << tcx)) * ((1 << log2d) / (4 << tcy));
-    return ncell <= 256 ? 1 : ncell / 256;
+    return ncell <= OCT_CELLS_PER_WARP ? 1 : ncell / OCT_CELLS_PER_WARP;
 }
 
 template <int LD, int TX, int TY, int BLK>

@@ -130,13 +130,41 @@ __device__ __forceinline__ void flip_links(uint32_t* Sb, uint32_t i, bool up)
     B[+4 * SH::P + 2] = v0;         // north neighbour's S link = sigma_y(x,y+1)
 }
 
-// The collective single-hit steps of one domain sweep (:168-174).  ALWAYS: the acceptance threshold of the only live direction is 65536 (p = 1 or q = 1),
-// so the r16 comparison is dropped.
-template <class SH, int BLK, bool ALWAYS>
+// Acceptance rule of one launch.  ONEDIR: only one of p, q is non-zero (always so for the sync variant),
+// so a single entry pattern is tested and the stored values are launch constants; ALWAYS: that live
+// threshold is 65536 (p = 1 or q = 1) and the 16-bit comparison is dropped as well.
+template <bool ONEDIR, bool ALWAYS>
+struct Rule {
+    uint32_t P16, Q16, target, T16;
+    bool dep;
+    __device__ __forceinline__ Rule(uint32_t p16, uint32_t q16)
+        : P16(p16), Q16(q16), target(q16 == 0u ? kEntryMin : kEntryMax), T16(q16 == 0u ? p16 : q16), dep(q16 == 0u) {}
+    // decision for entry value e and attempt word w: 0 nothing, +1 deposit, -1 remove
+    __device__ __forceinline__ int decide(uint32_t e, uint32_t w) const
+    {
+        if constexpr (ONEDIR) {
+            bool acc = e == target;
+            if constexpr (!ALWAYS) acc = acc && (w >> 16) < T16;
+            return acc ? (dep ? 1 : -1) : 0;
+        } else {
+            const uint32_t r16 = w >> 16;
+            return (e == kEntryMin && r16 < P16) ? 1 : ((e == kEntryMax && r16 < Q16) ? -1 : 0);
+        }
+    }
+    template <class SH>
+    __device__ __forceinline__ void apply(uint32_t* Sb, uint32_t i, int d) const
+    {
+        if constexpr (ONEDIR) { if (d != 0) flip_links<SH>(Sb, i, dep); }
+        else { if (d != 0) flip_links<SH>(Sb, i, d > 0); }
+    }
+};
+
+// The collective single-hit steps of one domain sweep (:168-174).
+template <class SH, int BLK, bool ONEDIR, bool ALWAYS>
 __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint32_t* __restrict__ BT, uint32_t tg, int grp,
                                          uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16)
 {
-    constexpr int CX = SH::CX, CY = SH::CY, D = SH::D, G = SH::G, CPT = SH::CPT;
+    constexpr int CX = SH::CX, CY = SH::CY, G = SH::G, CPT = SH::CPT;
     constexpr uint32_t LOG2NCX = 0 + (SH::NCX == 1 ? 0 : SH::NCX == 2 ? 1 : SH::NCX == 4 ? 2 : SH::NCX == 8 ? 3 : SH::NCX == 16 ? 4 : 5);
     static_assert((1 << LOG2NCX) == SH::NCX, "NCX must be a power of two <= 32");
     // x in bits 0-7, y in bits 8-15 of one register: the attempt word, the block-step word and the cell
@@ -149,9 +177,7 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
         const uint32_t c = tg + j * G;
         cellc[j] = ((c & (SH::NCX - 1)) * CX) | (((c >> LOG2NCX) * CY) << 8);
     }
-    // sync variant: exactly one direction is live (p*q == 0)
-    const bool dep = Q16 == 0u;
-    const uint32_t target = dep ? kEntryMin : kEntryMax, T16 = dep ? P16 : Q16;
+    const Rule<ONEDIR, ALWAYS> rule(P16, Q16);
 
 #pragma unroll 1
     for (uint32_t k4 = 0; k4 < (uint32_t)(SH::NSTEP / 4); ++k4) {
@@ -169,19 +195,17 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
                 // "ignoring borders" (:174) made order-free (R16): all cells decide on the state at the start
                 // of the step, then all accepted updates are carried out
                 const uint32_t sc = Bw & FM;
-                bool acc[CPT];
+                int dec[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
                     const uint32_t v = (w & FM) + cellc[j] + sc;
                     idx[j] = site_index<SH>(v);
-                    acc[j] = Sb[idx[j]] == target;
-                    if constexpr (!ALWAYS) acc[j] = acc[j] && (w >> 16) < T16;
+                    dec[j] = rule.decide(Sb[idx[j]], w);
                 }
                 group_sync<SH::WPD, SH::DPB>(grp);
 #pragma unroll
-                for (int j = 0; j < CPT; ++j)
-                    if (acc[j]) flip_links<SH>(Sb, idx[j], dep);
+                for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
                 group_sync<SH::WPD, SH::DPB>(grp);
             } else if constexpr (BLK == kBlkDelayed) {
                 // delayed borders (:174): bulk, then edges, then corners (R15)
@@ -196,27 +220,26 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
                 }
 #pragma unroll
                 for (uint32_t phase = 0; phase < 3; ++phase) {
+                    int dec[CPT];                    // cells of one phase never touch common links (R15): loads first
 #pragma unroll
-                    for (int j = 0; j < CPT; ++j)
-                        if (cls[j] == phase) {
-                            const uint32_t e = Sb[idx[j]], r16 = rw[j][kk] >> 16;
-                            if (e == kEntryMin && r16 < P16) flip_links<SH>(Sb, idx[j], true);
-                            else if (e == kEntryMax && r16 < Q16) flip_links<SH>(Sb, idx[j], false);
-                        }
+                    for (int j = 0; j < CPT; ++j) dec[j] = cls[j] == phase ? rule.decide(Sb[idx[j]], rw[j][kk]) : 0;
+#pragma unroll
+                    for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
                     group_sync<SH::WPD, SH::DPB>(grp);
                 }
             } else {
-                // block-layer DT (:170): one random quadrant of every cell per step (R17)
+                // block-layer DT (:170): one random quadrant of every cell per step (R17).  The cells of a step
+                // cannot interact, so all loads go first and the stores follow (no load waits behind a store)
                 const uint32_t qc = (((Bw >> 16) & 1u) * (CX / 2)) | ((((Bw >> 17) & 1u) * (CY / 2)) << 8);
+                int dec[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
-                    const uint32_t v = (w & FM) + cellc[j] + qc;
-                    const uint32_t i = site_index<SH>(v);
-                    const uint32_t e = Sb[i], r16 = w >> 16;
-                    if (e == kEntryMin && r16 < P16) flip_links<SH>(Sb, i, true);
-                    else if (e == kEntryMax && r16 < Q16) flip_links<SH>(Sb, i, false);
+                    idx[j] = site_index<SH>((w & FM) + cellc[j] + qc);
+                    dec[j] = rule.decide(Sb[idx[j]], w);
                 }
+#pragma unroll
+                for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
                 group_sync<SH::WPD, SH::DPB>(grp);
             }
         }
@@ -308,13 +331,12 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
     }
 
     // ---- a4-a6: collective single-hit steps (:168) ---------------------------------------------
-    if constexpr (BLK == kBlkSync) {
-        const uint32_t T16 = P.Q16 == 0u ? P.P16 : P.Q16;
-        if (T16 == 65536u) run_steps<SH, BLK, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
-        else               run_steps<SH, BLK, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
-    } else {
-        run_steps<SH, BLK, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
-    }
+    // launch-uniform specialisation of the acceptance rule (the sync variant is only used with p*q = 0, R16)
+    const bool onedir = BLK == kBlkSync || P.P16 == 0u || P.Q16 == 0u;
+    const uint32_t T16 = P.Q16 == 0u ? P.P16 : P.Q16;
+    if (onedir && T16 == 65536u) run_steps<SH, BLK, true, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
+    else if (onedir)             run_steps<SH, BLK, true, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
+    else if constexpr (BLK != kBlkSync) run_steps<SH, BLK, false, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
     // every variant of run_steps ends with a group barrier: the entries are final here
 
     // ---- a7: stage-out (:164): whole packed words of the window ---------------------------------
