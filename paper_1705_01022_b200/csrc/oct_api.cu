@@ -88,7 +88,7 @@ SweepLaunch make_launch()
 #define OCT_SHAPES(X)                                                      \
     X(5, 0, 0) X(5, 1, 1) X(5, 2, 2)                                       \
     X(6, 0, 0) X(6, 1, 1) X(6, 2, 2) X(6, 2, 1) X(6, 3, 1) X(6, 1, 3)      \
-    X(7, 0, 0) X(7, 1, 1) X(7, 2, 2) X(7, 2, 1)                            \
+    X(7, 0, 0) X(7, 1, 1) X(7, 2, 2) X(7, 2, 1) X(7, 3, 2) X(7, 4, 1)      \
     X(8, 1, 1) X(8, 2, 2) X(8, 2, 1) X(8, 3, 2) X(8, 4, 1)
 
 bool find_launch(int ld, int tx, int ty, int blk, SweepLaunch* out)
@@ -120,7 +120,7 @@ SweepLaunch make_links_launch()
 // B the alternative work split of the two headline shapes
 #define OCT_LINK_SHAPES_A(X)                                                         \
     X(5, 0, 0, 1, 4) X(6, 0, 0, 4, 1) X(6, 1, 1, 1, 4) X(6, 2, 1, 1, 4)              \
-    X(7, 0, 0, 8, 1) X(7, 1, 1, 8, 1) X(7, 2, 2, 2, 1) X(7, 2, 1, 4, 1)
+    X(7, 0, 0, 8, 1) X(7, 1, 1, 8, 1) X(7, 2, 2, 2, 1) X(7, 2, 1, 4, 1) X(7, 3, 2, 1, 1) X(7, 4, 1, 1, 1)
 #define OCT_LINK_SHAPES_B(X) X(6, 1, 1, 2, 2) X(7, 1, 1, 4, 1)
 
 bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, SweepLaunch* out)

@@ -65,6 +65,9 @@ SMALL = [
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 7), 1.0, 0.0, 6),
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 0, 0), 1.0, 0.0, 4),         # 4 warps per domain
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 2, 2), 0.9, 0.1, 4),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 3, 2), 1.0, 0.0, 3),         # Fig. 4 cell shapes at D = 128
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 7, 4, 1), 1.0, 0.0, 3),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 4, 1), 0.8, 0.2, 2),
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 1.0, 0.0, 6),               # D = 256: 4 warps, named CTA barrier
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 0.9, 0.1, 4),
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 8), 1.0, 0.0, 4),
@@ -217,6 +220,22 @@ def test_config2_shape_mixed_rates_L4096_prefix():
     orc.sweep(2, cfg.p, cfg.q, cfg.scheme); sim.oct_sweep(2, cfg.p, cfg.q, cfg.scheme)
     compare_state(sim, orc, check_heights=False)
     sim.close(); orc.close()
+
+
+def test_degenerate_calls_change_nothing():
+    """p = q = 0 (no update can be accepted) and n_mcs = 0 leave the lattice and the counters alone; the clock
+    advances only by the sweeps actually run.  Every kernel."""
+    for k in KERNELS.values():
+        for code in (wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6), wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6)):
+            sim = binding.Sim(256, 4)
+            sim.oct_set_option(binding.OCT_OPT_KERNEL, k)
+            sim.oct_sweep(3, 1.0, 0.0, code)
+            before, cnt = sim.oct_export().copy(), sim.oct_counters()
+            sim.oct_sweep(0, 1.0, 0.0, code)
+            assert sim.oct_mcs() == 3
+            sim.oct_sweep(2, 0.0, 0.0, code)
+            assert sim.oct_mcs() == 5 and (sim.oct_export() == before).all() and sim.oct_counters() == cnt
+            sim.close()
 
 
 def test_invalid_calls_are_rejected_without_side_effects():
