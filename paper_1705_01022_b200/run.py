@@ -15,9 +15,25 @@ from __future__ import annotations
 import argparse
 import json
 import math
+import sys
 import time
 
 from . import binding, workloads as wl
+
+
+def _strip(argv, flags):
+    """argv without the given `--flag value` pairs"""
+    out, skip = [], False
+    for a in argv:
+        if skip:
+            skip = False
+        elif a in flags:
+            skip = True
+        elif any(a.startswith(f + "=") for f in flags):
+            pass
+        else:
+            out.append(a)
+    return out
 
 
 def log_grid(t_max: int, per_decade: int, t_min: int = 1):
@@ -38,6 +54,32 @@ def eff_exponent(e1, t1, e0, t0):
     return math.log(e1 / e0) / math.log(t1 / t0)
 
 
+def ensemble_mean(runs, keys=("w2", "mean_h", "c_h", "c_s")):
+    """Mean and standard error over independent runs (seeds) of the per-run observables, grid point by grid
+    point -- the paper's ensemble average (R8: <.> inside a run is spatial, the sample mean
+    over runs is formed afterwards).  `runs` = list of row lists sharing one time grid."""
+    out = []
+    for rows in zip(*runs):
+        t = rows[0]["t"]
+        assert all(r["t"] == t for r in rows)
+        rec = {"t": t, "n": len(rows)}
+        for k in keys:
+            vals = [r[k] for r in rows if k in r]
+            if len(vals) != len(rows):
+                continue
+            m = sum(vals) / len(vals)
+            rec[k] = m
+            rec[k + "_sem"] = math.sqrt(sum((v - m) ** 2 for v in vals) / (len(vals) * (len(vals) - 1))) if len(vals) > 1 else None
+        out.append(rec)
+    prev = None
+    for r in out:                                                # Eq. (8) on the ensemble means
+        if prev is not None and r["t"] > 1:
+            e = eff_exponent(r["w2"], r["t"], prev["w2"], prev["t"])
+            r["beta_eff"] = None if e is None else e / 2
+        prev = r
+    return out
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__.split("\n")[0])
     ap.add_argument("--L", type=int, default=1 << 16)
@@ -46,6 +88,7 @@ def main(argv=None):
     ap.add_argument("--p", type=float, default=1.0)
     ap.add_argument("--q", type=float, default=0.0)
     ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--seeds", type=int, default=1, help="ensemble: run seeds seed .. seed+seeds-1 one after the other and average")
     ap.add_argument("--log2D", type=int, default=6)
     ap.add_argument("--tcx", type=int, default=1)
     ap.add_argument("--tcy", type=int, default=1)
@@ -54,6 +97,19 @@ def main(argv=None):
     ap.add_argument("--per-decade", type=int, default=8)
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
+    if args.seeds > 1:
+        runs = []
+        for sd in range(args.seed, args.seed + args.seeds):
+            sub = list(argv if argv is not None else sys.argv[1:])
+            one = main(_strip(sub, ("--seeds", "--seed", "--out")) + ["--seed", str(sd)])
+            runs.append(one["rows"])
+        ens = ensemble_mean(runs)
+        for r in ens:
+            print("ensemble " + " ".join(f"{k}={v:.6g}" if isinstance(v, float) else f"{k}={v}" for k, v in r.items()))
+        if args.out:
+            with open(args.out, "w") as f:
+                json.dump({"seeds": list(range(args.seed, args.seed + args.seeds)), "ensemble": ens}, f, indent=1)
+        return {"ensemble": ens}
 
     import torch
     L, N = args.L, args.L * args.L

@@ -21,3 +21,15 @@ def test_effective_exponent_recovers_a_power_law():
         assert run.eff_exponent(f(t1), t1, f(t0), t0) == pytest.approx(0.4828, rel=1e-12)
     assert run.eff_exponent(1.0, 10, 0.0, 5) is None and run.eff_exponent(1.0, 5, 1.0, 5) is None
     assert math.isclose(run.eff_exponent(0.5, 4, 1.0, 2), -1.0)
+
+
+def test_ensemble_mean_and_standard_error():
+    runs = [[{"t": 1, "w2": 1.0, "mean_h": 0.5}, {"t": 10, "w2": 4.0, "mean_h": 5.0}],
+            [{"t": 1, "w2": 3.0, "mean_h": 0.5}, {"t": 10, "w2": 6.0, "mean_h": 7.0}]]
+    e = run.ensemble_mean(runs)
+    assert [r["t"] for r in e] == [1, 10] and e[0]["n"] == 2
+    assert e[0]["w2"] == 2.0 and e[0]["w2_sem"] == pytest.approx(1.0)        # sqrt(((1)^2+(1)^2)/(2*1))
+    assert e[1]["w2"] == 5.0 and e[1]["mean_h_sem"] == pytest.approx(1.0)
+    assert e[1]["beta_eff"] == pytest.approx(math.log(5.0 / 2.0) / math.log(10.0) / 2)
+    assert "c_h" not in e[0]
+    assert run._strip(["--L", "64", "--seeds", "3", "--seed=2", "--out", "x"], ("--seeds", "--seed", "--out")) == ["--L", "64"]
