@@ -23,7 +23,7 @@ _LIB = os.path.join(_HERE, "liboct_oracle.so")
 
 # scheme encoding of include/oct.h (restated, not shared): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16
 DEV_DTR, DEV_DT, DEV_DB, DEV_CDB = 0, 1, 2, 3
-BLK_DB, BLK_DB_DELAYED, BLK_DT = 0, 1, 2
+BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR = 0, 1, 2, 3
 
 
 def scheme(dev: int, blk: int, log2D: int, tcx: int = 1, tcy: int = 1) -> int:

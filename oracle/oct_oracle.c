@@ -11,7 +11,7 @@
  *   - true random-sequential dynamics  :15/:44, 1 MCS = L^2 attempts :106               -> orc_sweep_rs
  *   - device-layer DD: DB/cDB          Sec. 3.0.1 :133-140, :166                         -> orc_sweep_dd
  *                      DT, DTr         Sec. 3.0.2 :142-146, Sec. 3.0.3 :148-150          -> orc_sweep_dd
- *   - block-layer single-hit DB / DT   Sec. 3.1 :168-174                                 -> domain_sweep
+ *   - block-layer single-hit DB / DT   Sec. 3.1 :168-174; DT with moving origin (DTr) :234 -> domain_sweep
  *   - roughness W^2, autocorr C_h      Eq. (3) :61, Eq. (6) :92-98                       -> orc_sums, orc_autocorr_sums
  *   - slope (lattice-gas) autocorr C_s :85-88 (unnumbered equation before Eq. (6))       -> orc_slope_autocorr_sums
  *   - RNG (paper silent)               Philox4x32-10, Salmon et al. SC'11; keying = DESIGN.md R19
@@ -242,7 +242,7 @@ int orc_sweep_rs(orc_state *s, uint64_t n_mcs, double p, double q)
 
 /* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16   (include/oct.h) */
 enum { DEV_DTR = 0, DEV_DT = 1, DEV_DB = 2, DEV_CDB = 3 };
-enum { BLK_DB_AUTO = 0, BLK_DB_DELAYED = 1, BLK_DT = 2 };
+enum { BLK_DB_AUTO = 0, BLK_DB_DELAYED = 1, BLK_DT = 2, BLK_DTR = 3 };
 
 /* tiny xorshift used ONLY by the order-shuffling test hook */
 static uint64_t xs64(uint64_t *st) { uint64_t v = *st; v ^= v << 13; v ^= v >> 7; v ^= v << 17; return *st = v; }
@@ -288,11 +288,17 @@ static int domain_sweep(orc_state *s, uint32_t set, uint32_t dom, uint32_t gx, u
         for (uint32_t c = 0; c < ncell; ++c) {
             const uint32_t a = c % ncx, b = c / ncx, w = wcache[4 * c + (k & 3)];
             uint32_t x, y; int cls;
-            if (blk == BLK_DT) {                       /* :170, random quadrant per step */
+            if (blk == BLK_DT || blk == BLK_DTR) {     /* :170, random quadrant per step */
                 const uint32_t Q = (B >> 16) & 3u;
                 const uint32_t lx = w & (cx / 2 - 1), ly = (w >> 8) & (cy / 2 - 1);
                 x = a * cx + (Q & 1u) * (cx / 2) + lx;
                 y = b * cy + (Q >> 1) * (cy / 2) + ly;
+                if (blk == BLK_DTR) {                  /* :234 "DTrDTr": the block-layer origin also moves
+                                                          after each collective update (R26): the
+                                                          same origin draw as block-layer DB, cells wrap (R14) */
+                    x = (x + (B & (cx - 1))) & (D - 1);
+                    y = (y + ((B >> 8) & (cy - 1))) & (D - 1);
+                }
                 cls = -1;
             } else {                                   /* :172, DB with random origin per step */
                 const uint32_t ox = B & (cx - 1), oy = (B >> 8) & (cy - 1);
@@ -308,7 +314,7 @@ static int domain_sweep(orc_state *s, uint32_t set, uint32_t dom, uint32_t gx, u
         }
         if (shuf) shuffle_u32(order, ncell, shuf);
 
-        if (blk == BLK_DT) {
+        if (blk == BLK_DT || blk == BLK_DTR) {
             for (uint32_t i = 0; i < ncell; ++i) {
                 const attempt_t *A = &att[order[i]];
                 int d = A->dead ? 0 : orc_attempt(s, A->X, A->Y, A->r16, P16, Q16);
@@ -366,10 +372,10 @@ int orc_check_scheme(uint32_t L, uint32_t scheme)
 {
     const uint32_t dev = scheme & 15u, blk = (scheme >> 4) & 15u, tcx = (scheme >> 8) & 15u,
                    tcy = (scheme >> 12) & 15u, lD = (scheme >> 16) & 31u;
-    if (dev > 3 || blk > 2 || lD < 3 || lD > 12) return -1;
+    if (dev > 3 || blk > 3 || lD < 3 || lD > 12) return -1;
     const uint32_t D = 1u << lD, cx = 4u << tcx, cy = 4u << tcy;
     if (cx > 64 || cy > 64 || cx > D || cy > D) return -1;
-    if (blk == BLK_DT && (tcx < 1 || tcy < 1)) return -1;             /* :182 smallest TC=1,1 for DT */
+    if ((blk == BLK_DT || blk == BLK_DTR) && (tcx < 1 || tcy < 1)) return -1;   /* :182 smallest TC=1,1 for DT */
     if (!is_pow2(L)) return -1;
     if ((dev == DEV_DTR || dev == DEV_DT) ? (L < 2 * D) : (L < D)) return -1;
     const uint64_t ntile = (dev <= DEV_DT) ? (uint64_t)(L / (2 * D)) * (L / (2 * D)) : (uint64_t)(L / D) * (L / D);

@@ -13,7 +13,7 @@ import numpy as np
 import pytest
 
 import oracle
-from oracle import BLK_DB, BLK_DB_DELAYED, BLK_DT, DEV_CDB, DEV_DB, DEV_DT, DEV_DTR, Oracle, scheme
+from oracle import BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR, DEV_CDB, DEV_DB, DEV_DT, DEV_DTR, Oracle, scheme
 
 
 def run_traced(L, seed, code, n_mcs, p=1.0, q=0.0, t0=0):
@@ -127,6 +127,49 @@ def test_dt_block_layer_trace(code):
     o.close()
 
 
+@pytest.mark.parametrize("code", [scheme(DEV_DTR, BLK_DTR, 5), scheme(DEV_DTR, BLK_DTR, 5, 2, 1)])
+def test_dtr_block_layer_trace(code):
+    """Block-layer DTr ("DTrDTr", R26): block-layer DT whose origin moves after each collective
+    update.  Per step all cells select inside one common quadrant (as DT) of their cell displaced by one
+    common origin (as DB) with wrap inside the domain; every cell is hit once per step, the origins are
+    uniform on [0,cx) x [0,cy), and with origin (0,0) the selection is exactly DT's."""
+    L, seed = 64, 9
+    D, cx, cy = dims(code)
+    o, tr = run_traced(L, seed, code, 2)
+    assert len(tr) == 2 * L * L
+    origins = []
+    for t in (0, 1):
+        Ox, Oy, perm = oracle.mcs_control(seed, t, L, DEV_DTR)
+        rec = tr[tr["t"] == t]
+        nt = L // (2 * D)
+        for s in range(4):
+            for dom in range(nt * nt):
+                rd = rec[(rec["set"] == s) & (rec["dom"] == dom)]
+                gx = (Ox + 2 * D * (dom % nt) + (s & 1) * D) % L
+                gy = (Oy + 2 * D * (dom // nt) + (s >> 1) * D) % L
+                lx, ly = (rd["x"].astype(np.int64) - gx) % L, (rd["y"].astype(np.int64) - gy) % L
+                assert (lx < D).all() and (ly < D).all()
+                a, b = rd["cell"] % (D // cx), rd["cell"] // (D // cx)
+                for k in range(cx * cy):
+                    m = rd["k"] == k
+                    assert m.sum() == (D // cx) * (D // cy) and len(set(rd["cell"][m].tolist())) == m.sum()
+                    # offsets from the cells' own corners, modulo the domain: all inside ONE window of
+                    # (cx/2) x (cy/2) sites = quadrant corner + common origin
+                    ux, uy = (lx[m] - a[m] * cx) % D, (ly[m] - b[m] * cy) % D
+                    for u, half, full in ((ux, cx // 2, cx), (uy, cy // 2, cy)):
+                        starts = [s0 for s0 in range(0, 2 * full) if all(((int(v) - s0) % D) < half for v in u)]
+                        assert starts, "cells of one step do not share a quadrant window"
+                    origins.append((int(ux.min()), int(uy.min())))
+    # the windows start anywhere in [0, cx + cx/2): quadrant offset {0, cx/2} + origin [0, cx)
+    xs = np.array([v[0] for v in origins]); ys = np.array([v[1] for v in origins])
+    assert xs.max() >= cx and ys.max() >= cy // 2 and xs.min() < 4 and ys.min() < 4
+    # against plain DT: identical attempts whenever the drawn origin is (0,0); different otherwise
+    o_dt, tr_dt = run_traced(L, seed, (code & ~0xF0) | (BLK_DT << 4), 2)
+    same = (tr["x"] == tr_dt["x"]) & (tr["y"] == tr_dt["y"])
+    assert 0 < same.mean() < 0.2
+    o.close(); o_dt.close()
+
+
 @pytest.mark.parametrize("dev,w", [(DEV_DB, 5), (DEV_CDB, 1)])
 def test_dead_border_device_layer(dev, w):
     L, seed, code = 128, 17, scheme(dev, BLK_DB, 5)
@@ -190,6 +233,7 @@ ORDER_CASES = [
     (scheme(DEV_DB, BLK_DB, 5), 0.9, 0.1), (scheme(DEV_CDB, BLK_DB, 5), 1.0, 0.0),
     (scheme(DEV_DB, BLK_DT, 5), 1.0, 0.0), (scheme(DEV_DTR, BLK_DB, 5, 2, 2), 0.9, 0.1),
     (scheme(DEV_DTR, BLK_DB, 5, 0, 0), 0.5, 0.5), (scheme(DEV_DTR, BLK_DB, 6, 3, 1), 1.0, 0.0),
+    (scheme(DEV_DTR, BLK_DTR, 5), 0.6, 0.4), (scheme(DEV_DTR, BLK_DTR, 5, 2, 1), 1.0, 0.0),
 ]
 
 

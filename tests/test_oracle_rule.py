@@ -207,6 +207,8 @@ CASES = [
     (scheme(DEV_DTR, BLK_DB, 6, 3, 1), 0.5, 0.5),
     (scheme(DEV_DTR, BLK_DT, 6, 1, 3), 1.0, 0.0),
     (scheme(DEV_DTR, BLK_DB, 5, 0, 0), 0.5, 0.5),
+    (scheme(DEV_DTR, 3, 5), 0.7, 0.3),            # block-layer DTr
+    (scheme(DEV_DB, 3, 5, 2, 1), 1.0, 0.0),
 ]
 
 
