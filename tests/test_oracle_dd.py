@@ -307,7 +307,8 @@ def test_invalid_schemes_are_rejected():
     assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DT, 5, 0, 1)) != 0  # DT needs TC >= 1,1 (:182)
     assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DB, 3, 2, 0)) != 0  # cell larger than domain
     assert lib.orc_check_scheme(96, scheme(DEV_DTR, BLK_DB, 4)) != 0         # L not a power of two
-    assert lib.orc_check_scheme(128, scheme(4, BLK_DB, 5)) != 0 and lib.orc_check_scheme(128, scheme(0, 3, 5)) != 0
+    assert lib.orc_check_scheme(128, scheme(4, BLK_DB, 5)) != 0 and lib.orc_check_scheme(128, scheme(0, 4, 5)) != 0
+    assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DTR, 5, 0, 1)) != 0 and lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DTR, 5)) == 0
 
 
 def test_filtered_run_reproduces_the_interior():
