@@ -58,12 +58,13 @@ enum {
  *                                                 borders otherwise (:174, R16)
  *                                          1 DB   delayed borders forced
  *                                          2 DT   one random quadrant of every cell per step (:170)
+ *                                          3 DTr  DT whose cell origin also moves every step ("DTrDTr", :234, R26)
  *   tcx,tcy: log2 of the thread-cell edge in words of 4 sites, "TC=tcx,tcy" (:180); cell = 4<<tc sites
  *   log2D  : log2 of the device-layer domain edge D in sites (the sub-tile one worker sweeps)       */
 #define OCT_SCHEME(dev, blk, tcx, tcy, log2D) \
     ((dev) | ((blk) << 4) | ((tcx) << 8) | ((tcy) << 12) | ((log2D) << 16))
 enum { OCT_DEV_DTR = 0, OCT_DEV_DT = 1, OCT_DEV_DB = 2, OCT_DEV_CDB = 3 };
-enum { OCT_BLK_DB = 0, OCT_BLK_DB_DELAYED = 1, OCT_BLK_DT = 2 };
+enum { OCT_BLK_DB = 0, OCT_BLK_DB_DELAYED = 1, OCT_BLK_DT = 2, OCT_BLK_DTR = 3 };
 
 /* Sizes of the caller-allocated device buffers for an L x L lattice (0 if L is invalid). */
 size_t oct_lattice_bytes(uint32_t L);      /* L*L/4                                                  */
@@ -88,7 +89,7 @@ int oct_set_state(oct_ctx*, uint64_t t_mcs, int64_t h00, int64_t net, void* stre
  * lasts (1 - N_border/N) MCS of physical time (Eq. (9) :137, R9; see oct_time_per_sweep).
  * oct_sweep(a) followed by oct_sweep(b) equals oct_sweep(a+b).
  * Errors (nothing is enqueued): EINVAL for p,q outside [0,1], unknown dev/blk, cell larger than the
- * domain, blk=DT with tc<1 (:182), L < 2D, D outside {32,64,128,256} or a (D,TC) pair the library was
+ * domain, blk=DT/DTr with tc<1 (:182), L < 2D, D outside {32,64,128,256} or a (D,TC) pair the library was
  * not built for, t+n_mcs > 2^32-1.  ECUDA: a launch failed (text via oct_last_error). */
 int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* stream);
 

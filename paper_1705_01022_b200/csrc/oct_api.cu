@@ -153,14 +153,15 @@ int check_scheme(uint32_t L, int scheme)
     if (scheme < 0 || !valid_L(L)) return OCT_EINVAL;
     const SchemeFields f = split_scheme(scheme);
     if ((static_cast<uint32_t>(scheme) >> 21) != 0) return OCT_EINVAL;
-    if (f.dev > 3 || f.blk > 2) return OCT_EINVAL;
+    if (f.dev > 3 || f.blk > 3) return OCT_EINVAL;
     if (f.log2D < 5 || f.log2D > 8) return OCT_EINVAL;
     const uint32_t D = 1u << f.log2D, cx = 4u << f.tcx, cy = 4u << f.tcy;
     if (cx > D || cy > D || cx > 64 || cy > 64) return OCT_EINVAL;
-    if (f.blk == OCT_BLK_DT && (f.tcx < 1 || f.tcy < 1)) return OCT_EINVAL;   // :182
+    const bool blk_dt = f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR;
+    if (blk_dt && (f.tcx < 1 || f.tcy < 1)) return OCT_EINVAL;   // :182
     if (L < 2 * D) return OCT_EINVAL;   // window (D/4+1 words) must not wrap onto itself
     SweepLaunch sl;
-    if (!find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, f.blk == OCT_BLK_DT ? kBlkDT : kBlkSync, &sl)) return OCT_EINVAL;
+    if (!find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk_dt ? kBlkDT : kBlkSync, &sl)) return OCT_EINVAL;
     return OCT_OK;
 }
 
@@ -261,7 +262,7 @@ int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* 
     if (c->t + n_mcs > 0xFFFFFFFFull || c->t + n_mcs < c->t) return OCT_EINVAL;
     const SchemeFields f = split_scheme(scheme);
     const uint32_t P16 = prob16(p), Q16 = prob16(q);
-    const int blk = f.blk == OCT_BLK_DT ? kBlkDT
+    const int blk = (f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR) ? kBlkDT
                   : (f.blk == OCT_BLK_DB_DELAYED || (P16 > 0 && Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
     SweepLaunch sl;
     // the link-entry kernel serves the tiled device layers on domains that fit shared memory unpacked;
@@ -281,6 +282,7 @@ int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* 
     SweepParams sp{};
     sp.lat = c->lat; sp.counters = c->counters(); sp.L = c->L; sp.log2L = c->log2L;
     sp.P16 = P16; sp.Q16 = Q16; sp.dev = f.dev; sp.ndom = ndom; sp.rk = c->rk;
+    sp.dtr_mask = f.blk == OCT_BLK_DTR ? ~0u : 0u;
     for (uint64_t i = 0; i < n_mcs; ++i) {
         sp.t = static_cast<uint32_t>(c->t);
         for (uint32_t si = 0; si < (tiled ? 4u : 1u); ++si) {   // :144 sync = kernel boundary after each set

@@ -34,6 +34,7 @@ struct SweepParams {
     uint32_t P16, Q16;              // acceptance thresholds, accept iff r16 < P16 (R18)
     uint32_t dev;                   // device-layer scheme
     uint32_t ndom;                  // domains in this launch
+    uint32_t dtr_mask;              // block-layer DT: 0; block-layer DTr (:234, R26): ~0 (the origin also moves)
     PhiloxRoundKeys rk;
 };
 
@@ -207,12 +208,14 @@ sweep_kernel(const __grid_constant__ SweepParams P)
             Attempt at[CPT];
             if constexpr (BLK == kBlkDT) {
                 // :170 one random quadrant for all cells of the block in this step (R17)
-                const uint32_t qx = ((Bw >> 16) & 1u) * (CX / 2), qy = ((Bw >> 17) & 1u) * (CY / 2);
+                // block-layer DTr (:234, R26) adds the per-step origin of block-layer DB, cells wrap (R14)
+                const uint32_t qx = ((Bw >> 16) & 1u) * (CX / 2) + (Bw & (CX - 1) & P.dtr_mask);
+                const uint32_t qy = ((Bw >> 17) & 1u) * (CY / 2) + ((Bw >> 8) & (CY - 1) & P.dtr_mask);
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t c = tg + j * G, w = rw[j][kk];
-                    const uint32_t x = (c & (SH::NCX - 1)) * CX + qx + (w & (CX / 2 - 1));
-                    const uint32_t y = (c >> LOG2NCX) * CY + qy + ((w >> 8) & (CY / 2 - 1));
+                    const uint32_t x = ((c & (SH::NCX - 1)) * CX + qx + (w & (CX / 2 - 1))) & (D - 1);
+                    const uint32_t y = ((c >> LOG2NCX) * CY + qy + ((w >> 8) & (CY / 2 - 1))) & (D - 1);
                     int dec = 0; uint32_t loc = 0;
                     const bool live = (!SH::PARTIAL || c < (uint32_t)SH::NCELL) && x < dead_lim && y < dead_lim;
                     if (live) dec = decide_at<SH>(S, x + offx, y + offy, w >> 16, P16, Q16, loc);

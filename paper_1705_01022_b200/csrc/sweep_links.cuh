@@ -162,7 +162,7 @@ struct Rule {
 // The collective single-hit steps of one domain sweep (:168-174).
 template <class SH, int BLK, bool ONEDIR, bool ALWAYS>
 __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint32_t* __restrict__ BT, uint32_t tg, int grp,
-                                         uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16)
+                                         uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16, uint32_t dtr_mask)
 {
     constexpr int CX = SH::CX, CY = SH::CY, G = SH::G, CPT = SH::CPT;
     constexpr uint32_t LOG2NCX = 0 + (SH::NCX == 1 ? 0 : SH::NCX == 2 ? 1 : SH::NCX == 4 ? 2 : SH::NCX == 8 ? 3 : SH::NCX == 16 ? 4 : 5);
@@ -230,7 +230,9 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
             } else {
                 // block-layer DT (:170): one random quadrant of every cell per step (R17).  The cells of a step
                 // cannot interact, so all loads go first and the stores follow (no load waits behind a store)
-                const uint32_t qc = (((Bw >> 16) & 1u) * (CX / 2)) | ((((Bw >> 17) & 1u) * (CY / 2)) << 8);
+                // (block-layer DTr, :234 / R26: plus the per-step origin of block-layer DB; site_index wraps, R14)
+                const uint32_t qc = ((((Bw >> 16) & 1u) * (CX / 2)) | ((((Bw >> 17) & 1u) * (CY / 2)) << 8))
+                                    + (Bw & dtr_mask & (uint32_t)((CX - 1) | ((CY - 1) << 8)));
                 int dec[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
@@ -334,9 +336,9 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
     // launch-uniform specialisation of the acceptance rule (the sync variant is only used with p*q = 0, R16)
     const bool onedir = BLK == kBlkSync || P.P16 == 0u || P.Q16 == 0u;
     const uint32_t T16 = P.Q16 == 0u ? P.P16 : P.Q16;
-    if (onedir && T16 == 65536u) run_steps<SH, BLK, true, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
-    else if (onedir)             run_steps<SH, BLK, true, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
-    else if constexpr (BLK != kBlkSync) run_steps<SH, BLK, false, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16);
+    if (onedir && T16 == 65536u) run_steps<SH, BLK, true, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask);
+    else if (onedir)             run_steps<SH, BLK, true, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask);
+    else if constexpr (BLK != kBlkSync) run_steps<SH, BLK, false, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask);
     // every variant of run_steps ends with a group barrier: the entries are final here
 
     // ---- a7: stage-out (:164): whole packed words of the window ---------------------------------

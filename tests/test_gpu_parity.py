@@ -45,6 +45,10 @@ SMALL = [
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB_DELAYED, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6), 1.0, 0.0, 12),
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6), 0.7, 0.3, 8),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 6), 1.0, 0.0, 8),              # "DTrDTr"
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 7, 2, 1), 0.7, 0.3, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 8), 1.0, 0.0, 3),
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DTR, 6), 0.6, 0.4, 4),
     (256, wl.scheme_code(wl.DEV_DT, wl.BLK_DB, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_DT, wl.BLK_DT, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 8),
