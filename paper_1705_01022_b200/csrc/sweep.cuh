@@ -1,11 +1,13 @@
-// Sweep kernel: one launch = one domain-set sweep of a DD scheme of arXiv 1705.01022 (Sec. 3).
+// Sweep kernel, bit-packed window: one launch = one domain-set sweep of a DD scheme of arXiv 1705.01022
+// (Sec. 3).  This is the general kernel (every device layer incl. the dead-border schemes, D up to 256);
+// sweep_links.cuh holds the faster link-entry kernel that serves DTr/DT for D <= 128.
 //
 // B200 mapping (differs from the paper's Kepler kernel):
 //   * a device-layer domain (D x D sites) is owned by a small *worker group* of WPD
-//     warps -- one single warp where the domain has <= 256 thread cells -- instead of one
+//     warps -- one single warp where the domain has <= 128 thread cells -- instead of one
 //     1024-thread block.  The block-layer thread cells (:168) are logical: each lane carries CPT cells
 //     per collective step (instruction-level parallelism), and the per-step synchronisation is
-//     __syncwarp (WPD = 1) or a named barrier over the group, never a whole-CTA barrier.
+//     __syncwarp (WPD = 1), a named barrier over the group, or the CTA barrier when the group is the CTA.
 //   * the domain window ((D/4+1)^2 words: D x D sites plus the +x / +y halo, :140, :164) is staged
 //     into shared memory in the lattice's own word alignment, odd pitch (:123 "padding by one word").
 //   * all random numbers are Philox4x32-10 words generated in registers (one call = 4 steps of one
