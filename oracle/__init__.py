@@ -22,7 +22,7 @@ _SRC = os.path.join(_HERE, "oct_oracle.c")
 _LIB = os.path.join(_HERE, "liboct_oracle.so")
 
 # scheme encoding of include/oct.h (restated, not shared): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16
-DEV_DTR, DEV_DT, DEV_DB, DEV_CDB = 0, 1, 2, 3
+DEV_DTR, DEV_DT, DEV_DB, DEV_CDB, DEV_DBH = 0, 1, 2, 3, 4
 BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR = 0, 1, 2, 3
 
 

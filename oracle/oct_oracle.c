@@ -9,7 +9,7 @@
  * What each part follows (PAPER.md line : section):
  *   - update rule                      Eq. (1) :27-34, Fig. 1 caption :50, :52, :140   -> orc_attempt
  *   - true random-sequential dynamics  :15/:44, 1 MCS = L^2 attempts :106               -> orc_sweep_rs
- *   - device-layer DD: DB/cDB          Sec. 3.0.1 :133-140, :166                         -> orc_sweep_dd
+ *   - device-layer DD: DB/cDB          Sec. 3.0.1 :133-140, :166; t_async = 1/2 :204-206 -> orc_sweep_dd
  *                      DT, DTr         Sec. 3.0.2 :142-146, Sec. 3.0.3 :148-150          -> orc_sweep_dd
  *   - block-layer single-hit DB / DT   Sec. 3.1 :168-174; DT with moving origin (DTr) :234 -> domain_sweep
  *   - roughness W^2, autocorr C_h      Eq. (3) :61, Eq. (6) :92-98                       -> orc_sums, orc_autocorr_sums
@@ -241,7 +241,7 @@ int orc_sweep_rs(orc_state *s, uint64_t n_mcs, double p, double q)
 /* ------------------------------------------------------------------------------- DD schemes */
 
 /* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16   (include/oct.h) */
-enum { DEV_DTR = 0, DEV_DT = 1, DEV_DB = 2, DEV_CDB = 3 };
+enum { DEV_DTR = 0, DEV_DT = 1, DEV_DB = 2, DEV_CDB = 3, DEV_DBH = 4 };
 enum { BLK_DB_AUTO = 0, BLK_DB_DELAYED = 1, BLK_DT = 2, BLK_DTR = 3 };
 
 /* tiny xorshift used ONLY by the order-shuffling test hook */
@@ -258,7 +258,7 @@ typedef struct { uint32_t X, Y; uint32_t r16; int cls; int dead; } attempt_t;
  * DxD domain; dead_w = device-layer dead-border width (0 for DT/DTr). */
 static int domain_sweep(orc_state *s, uint32_t set, uint32_t dom, uint32_t gx, uint32_t gy,
                         uint32_t D, uint32_t cx, uint32_t cy, int blk, uint32_t dead_w,
-                        uint32_t P16, uint32_t Q16, uint64_t *shuf)
+                        uint32_t P16, uint32_t Q16, uint64_t *shuf, uint32_t k_begin, uint32_t k_end)
 {
     const uint32_t key[2] = { (uint32_t)s->seed, (uint32_t)(s->seed >> 32) };
     const uint32_t ncx = D / cx, ncy = D / cy, ncell = ncx * ncy, nsteps = cx * cy, m = s->L - 1;
@@ -272,14 +272,15 @@ static int domain_sweep(orc_state *s, uint32_t set, uint32_t dom, uint32_t gx, u
     uint32_t *order  = (uint32_t *)malloc((size_t)ncell * sizeof(uint32_t));
     if (!wcache || !att || !dec || !order) { free(wcache); free(att); free(dec); free(order); return -3; }
 
-    for (uint32_t k = 0; k < nsteps; ++k) {
+    (void)nsteps;   /* a full sweep is k_begin = 0, k_end = cx*cy; DB with t_async = 1/2 runs half of it */
+    for (uint32_t k = k_begin; k < k_end; ++k) {
         /* block-step word B for (t, set, dom, k) */
         uint32_t bo[4], bctr[4] = { k >> 2, 0, c2b, (uint32_t)s->t };
         orc_philox4x32_10(bctr, key, bo);
         const uint32_t B = bo[k & 3];
 
         /* attempt word w for (t, set, dom, cell, k): one Philox call serves 4 consecutive steps */
-        if ((k & 3) == 0)
+        if ((k & 3) == 0 || k == k_begin)
             for (uint32_t c = 0; c < ncell; ++c) {
                 uint32_t cctr[4] = { k >> 2, c, c2c, (uint32_t)s->t };
                 orc_philox4x32_10(cctr, key, &wcache[4 * c]);
@@ -372,7 +373,7 @@ int orc_check_scheme(uint32_t L, uint32_t scheme)
 {
     const uint32_t dev = scheme & 15u, blk = (scheme >> 4) & 15u, tcx = (scheme >> 8) & 15u,
                    tcy = (scheme >> 12) & 15u, lD = (scheme >> 16) & 31u;
-    if (dev > 3 || blk > 3 || lD < 3 || lD > 12) return -1;
+    if (dev > 4 || blk > 3 || lD < 3 || lD > 12) return -1;
     const uint32_t D = 1u << lD, cx = 4u << tcx, cy = 4u << tcy;
     if (cx > 64 || cy > 64 || cx > D || cy > D) return -1;
     if ((blk == BLK_DT || blk == BLK_DTR) && (tcx < 1 || tcy < 1)) return -1;   /* :182 smallest TC=1,1 for DT */
@@ -415,28 +416,35 @@ int orc_sweep_dd(orc_state *s, uint64_t n_mcs, double p, double q, uint32_t sche
                     const uint32_t gx = (Ox + 2 * D * I + sx * D) & m, gy = (Oy + 2 * D * J + sy * D) & m;
                     if (s->filter_on && !(ring_meets(gx, D, s->fx0, s->fw, L) && ring_meets(gy, D, s->fy0, s->fh, L)))
                         continue;
-                    int rc = domain_sweep(s, set, dom, gx, gy, D, cx, cy, (int)blk, 0, P16, Q16, shuf);
+                    int rc = domain_sweep(s, set, dom, gx, gy, D, cx, cy, (int)blk, 0, P16, Q16, shuf, 0, cx * cy);
                     if (rc) { free(dorder); return rc; }
                 }
             }
             free(dorder);
         } else {
-            /* :135 dead border; :166 cDB = origin on the 4x4 word grid, border 1; DB = free origin, border 5 */
-            const uint32_t Ox = dev == DEV_CDB ? (G[0] & m & ~3u) : (G[0] & m);
-            const uint32_t Oy = dev == DEV_CDB ? (G[1] & m & ~3u) : (G[1] & m);
+            /* :135 dead border; :166 cDB = origin on the 4x4 word grid, border 1; DB = free origin, border 5.
+             * DBh (:204-206, R27): DB with t_async = 1/2 MCS -- two intervals per sweep, each with
+             * its own origin (global stream c0 = interval) and half of the collective steps. */
+            const uint32_t n_int = dev == DEV_DBH ? 2u : 1u;
             const uint32_t dead_w = dev == DEV_CDB ? 1u : 5u;
             const uint32_t nt = L / D;
             uint32_t *dorder = (uint32_t *)malloc((size_t)nt * nt * sizeof(uint32_t));
             if (!dorder) return -3;
-            for (uint32_t d = 0; d < nt * nt; ++d) dorder[d] = d;
-            if (shuf) shuffle_u32(dorder, nt * nt, shuf);
-            for (uint32_t di = 0; di < nt * nt; ++di) {
-                const uint32_t dom = dorder[di], I = dom % nt, J = dom / nt;
-                const uint32_t gx = (Ox + D * I) & m, gy = (Oy + D * J) & m;
-                if (s->filter_on && !(ring_meets(gx, D, s->fx0, s->fw, L) && ring_meets(gy, D, s->fy0, s->fh, L)))
-                    continue;
-                int rc = domain_sweep(s, 0, dom, gx, gy, D, cx, cy, (int)blk, dead_w, P16, Q16, shuf);
-                if (rc) { free(dorder); return rc; }
+            for (uint32_t iv = 0; iv < n_int; ++iv) {
+                if (iv > 0) { gctr[0] = iv; orc_philox4x32_10(gctr, key, G); }
+                const uint32_t Ox = dev == DEV_CDB ? (G[0] & m & ~3u) : (G[0] & m);
+                const uint32_t Oy = dev == DEV_CDB ? (G[1] & m & ~3u) : (G[1] & m);
+                const uint32_t k_begin = iv * (cx * cy / n_int), k_end = (iv + 1) * (cx * cy / n_int);
+                for (uint32_t d = 0; d < nt * nt; ++d) dorder[d] = d;
+                if (shuf) shuffle_u32(dorder, nt * nt, shuf);
+                for (uint32_t di = 0; di < nt * nt; ++di) {
+                    const uint32_t dom = dorder[di], I = dom % nt, J = dom / nt;
+                    const uint32_t gx = (Ox + D * I) & m, gy = (Oy + D * J) & m;
+                    if (s->filter_on && !(ring_meets(gx, D, s->fx0, s->fw, L) && ring_meets(gy, D, s->fy0, s->fh, L)))
+                        continue;
+                    int rc = domain_sweep(s, iv, dom, gx, gy, D, cx, cy, (int)blk, dead_w, P16, Q16, shuf, k_begin, k_end);
+                    if (rc) { free(dorder); return rc; }
+                }
             }
             free(dorder);
         }

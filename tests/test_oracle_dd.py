@@ -13,7 +13,7 @@ import numpy as np
 import pytest
 
 import oracle
-from oracle import BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR, DEV_CDB, DEV_DB, DEV_DT, DEV_DTR, Oracle, scheme
+from oracle import BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR, DEV_CDB, DEV_DB, DEV_DBH, DEV_DT, DEV_DTR, Oracle, scheme
 
 
 def run_traced(L, seed, code, n_mcs, p=1.0, q=0.0, t0=0):
@@ -193,6 +193,61 @@ def test_dead_border_device_layer(dev, w):
     o.close()
 
 
+def test_dead_border_half_sweep_intervals():
+    """DB with t_async = 1/2 MCS (R27): a sweep is two asynchronous intervals, each with its
+    own tiling origin and half of the collective steps, so every tile gets D^2/2 attempts per interval."""
+    L, seed, D, cx, cy, w = 128, 23, 32, 8, 8, 5
+    code = scheme(DEV_DBH, BLK_DB, 5)
+    o, tr = run_traced(L, seed, code, 2)
+    assert len(tr) == 2 * L * L                                       # still L^2 attempts per sweep (:106)
+    nt = L // D
+    moved = 0
+    for t in range(2):
+        rec = tr[tr["t"] == t]
+        halves = (rec[rec["k"] < cx * cy // 2], rec[rec["k"] >= cx * cy // 2])
+        assert len(halves[0]) == len(halves[1]) == L * L // 2
+        assert (halves[0]["set"] == 0).all() and (halves[1]["set"] == 1).all()      # the interval index keys the streams
+        origins = []
+        for iv, part in enumerate(halves):
+            # recover the interval's origin from any attempt of tile 0 / cell 0: x = O + (lx + ox) mod D ...
+            # simpler and stricter: there must be ONE origin (Ox, Oy) that puts every attempt of tile `dom`
+            # into that tile and every discarded attempt into the 5-wide border
+            cand = None
+            r0 = part[0]
+            for Ox in range(L):
+                if ((int(r0["x"]) - Ox) % L) // D == int(r0["dom"]) % nt:
+                    lx = (part["x"].astype(np.int64) - Ox) % L
+                    if ((lx // D) == part["dom"] % nt).all():
+                        bx = (lx % D) >= D - w
+                        cand = (Ox, bx) if cand is None else cand
+                        break
+            assert cand is not None
+            Ox, bx = cand
+            for Oy in range(L):
+                ly = (part["y"].astype(np.int64) - Oy) % L
+                if ((ly // D) == part["dom"] // nt).all():
+                    by = (ly % D) >= D - w
+                    break
+            else:
+                raise AssertionError("no y origin fits")
+            assert ((part["result"] == 2) == (bx | by)).all()
+            origins.append((Ox, Oy))
+            for dom in (0, nt * nt - 1):
+                assert (part["dom"] == dom).sum() == D * D // 2
+        Ox0, Oy0, _ = oracle.mcs_control(seed, t, L, DEV_DB)
+        assert origins[0] == (Ox0, Oy0)                                  # interval 0 = the plain DB draw (c0 = 0)
+        moved += origins[0] != origins[1]
+    assert moved == 2                                                     # the origin moves between the intervals
+    # the first interval of DBh is exactly the first half of a DB sweep
+    o_db, tr_db = run_traced(L, seed, scheme(DEV_DB, BLK_DB, 5), 1)
+    first = tr[(tr["t"] == 0) & (tr["k"] < cx * cy // 2)]
+    ref = tr_db[tr_db["k"] < cx * cy // 2]
+    # the oracle visits tile by tile, so compare as sets of (dom, cell, k, x, y)
+    key = lambda a: sorted(zip(a["dom"].tolist(), a["cell"].tolist(), a["k"].tolist(), a["x"].tolist(), a["y"].tolist()))
+    assert key(first) == key(ref)
+    o.close(); o_db.close()
+
+
 def test_origin_and_permutation_statistics():
     L = 1024
     ox, oy, perms = [], [], []
@@ -234,6 +289,7 @@ ORDER_CASES = [
     (scheme(DEV_DB, BLK_DT, 5), 1.0, 0.0), (scheme(DEV_DTR, BLK_DB, 5, 2, 2), 0.9, 0.1),
     (scheme(DEV_DTR, BLK_DB, 5, 0, 0), 0.5, 0.5), (scheme(DEV_DTR, BLK_DB, 6, 3, 1), 1.0, 0.0),
     (scheme(DEV_DTR, BLK_DTR, 5), 0.6, 0.4), (scheme(DEV_DTR, BLK_DTR, 5, 2, 1), 1.0, 0.0),
+    (scheme(DEV_DBH, BLK_DB, 5), 0.7, 0.3), (scheme(DEV_DBH, BLK_DT, 5), 1.0, 0.0),
 ]
 
 
@@ -307,7 +363,7 @@ def test_invalid_schemes_are_rejected():
     assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DT, 5, 0, 1)) != 0  # DT needs TC >= 1,1 (:182)
     assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DB, 3, 2, 0)) != 0  # cell larger than domain
     assert lib.orc_check_scheme(96, scheme(DEV_DTR, BLK_DB, 4)) != 0         # L not a power of two
-    assert lib.orc_check_scheme(128, scheme(4, BLK_DB, 5)) != 0 and lib.orc_check_scheme(128, scheme(0, 4, 5)) != 0
+    assert lib.orc_check_scheme(128, scheme(5, BLK_DB, 5)) != 0 and lib.orc_check_scheme(128, scheme(0, 4, 5)) != 0
     assert lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DTR, 5, 0, 1)) != 0 and lib.orc_check_scheme(128, scheme(DEV_DTR, BLK_DTR, 5)) == 0
 
 

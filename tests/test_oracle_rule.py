@@ -209,6 +209,7 @@ CASES = [
     (scheme(DEV_DTR, BLK_DB, 5, 0, 0), 0.5, 0.5),
     (scheme(DEV_DTR, 3, 5), 0.7, 0.3),            # block-layer DTr
     (scheme(DEV_DB, 3, 5, 2, 1), 1.0, 0.0),
+    (scheme(4, BLK_DB, 5), 0.8, 0.2),             # DB with t_async = 1/2
 ]
 
 
