@@ -52,6 +52,8 @@ enum {
  *                                          1 DT   double tiling, fixed origin         (:142-146)
  *                                          2 DB   dead border, free origin, width 5   (:133-140, :166)
  *                                          3 cDB  dead border, origin on the 4-site grid, width 1 (:166)
+ *                                          4 DBh  DB with t_async = 1/2 MCS: two intervals per sweep, each with
+ *                                                 its own origin and half of the collective steps (:204-206, R27)
  *   blk  (block layer, single-hit, Sec. 3.1 :168-174):
  *                                          0 DB   random cell origin per collective step; "ignoring
  *                                                 borders" when only one of p,q is non-zero, delayed
@@ -63,7 +65,7 @@ enum {
  *   log2D  : log2 of the device-layer domain edge D in sites (the sub-tile one worker sweeps)       */
 #define OCT_SCHEME(dev, blk, tcx, tcy, log2D) \
     ((dev) | ((blk) << 4) | ((tcx) << 8) | ((tcy) << 12) | ((log2D) << 16))
-enum { OCT_DEV_DTR = 0, OCT_DEV_DT = 1, OCT_DEV_DB = 2, OCT_DEV_CDB = 3 };
+enum { OCT_DEV_DTR = 0, OCT_DEV_DT = 1, OCT_DEV_DB = 2, OCT_DEV_CDB = 3, OCT_DEV_DBH = 4 };
 enum { OCT_BLK_DB = 0, OCT_BLK_DB_DELAYED = 1, OCT_BLK_DT = 2, OCT_BLK_DTR = 3 };
 
 /* Sizes of the caller-allocated device buffers for an L x L lattice (0 if L is invalid). */
@@ -85,7 +87,7 @@ int oct_set_state(oct_ctx*, uint64_t t_mcs, int64_t h00, int64_t net, void* stre
 /* n_mcs sweeps of the whole lattice (1 MCS = L^2 update attempts, :106) under DD scheme `scheme`,
  * deposition probability p at local minima and removal probability q at local maxima (Eq. (1)
  * :27-34; p,q in [0,1], quantised to 1/65536, R18).  DTr/DT: 4 kernel launches per MCS, one per domain
- * set, in the permutation drawn for that MCS (:144); DB/cDB: 1 launch per MCS, and one such sweep
+ * set, in the permutation drawn for that MCS (:144); DB/cDB: 1 launch per MCS (DBh: 2), and one such sweep
  * lasts (1 - N_border/N) MCS of physical time (Eq. (9) :137, R9; see oct_time_per_sweep).
  * oct_sweep(a) followed by oct_sweep(b) equals oct_sweep(a+b).
  * Errors (nothing is enqueued): EINVAL for p,q outside [0,1], unknown dev/blk, cell larger than the

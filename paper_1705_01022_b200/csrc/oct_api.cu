@@ -153,7 +153,7 @@ int check_scheme(uint32_t L, int scheme)
     if (scheme < 0 || !valid_L(L)) return OCT_EINVAL;
     const SchemeFields f = split_scheme(scheme);
     if ((static_cast<uint32_t>(scheme) >> 21) != 0) return OCT_EINVAL;
-    if (f.dev > 3 || f.blk > 3) return OCT_EINVAL;
+    if (f.dev > 4 || f.blk > 3) return OCT_EINVAL;
     if (f.log2D < 5 || f.log2D > 8) return OCT_EINVAL;
     const uint32_t D = 1u << f.log2D, cx = 4u << f.tcx, cy = 4u << f.tcy;
     if (cx > D || cy > D || cx > 64 || cy > 64) return OCT_EINVAL;
@@ -285,7 +285,8 @@ int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* 
     sp.dtr_mask = f.blk == OCT_BLK_DTR ? ~0u : 0u;
     for (uint64_t i = 0; i < n_mcs; ++i) {
         sp.t = static_cast<uint32_t>(c->t);
-        for (uint32_t si = 0; si < (tiled ? 4u : 1u); ++si) {   // :144 sync = kernel boundary after each set
+        const uint32_t n_launch = tiled ? 4u : (f.dev == OCT_DEV_DBH ? 2u : 1u);   // DBh: two intervals (R27)
+        for (uint32_t si = 0; si < n_launch; ++si) {   // :144 sync = kernel boundary after each set
             sp.si = si;
             sl.kern<<<grid, sl.threads, sl.smem, st>>>(sp);
             c->launches++;
@@ -466,7 +467,7 @@ double oct_time_per_sweep(uint32_t L, int scheme)
     if (check_scheme(L, scheme) != OCT_OK) return 0.0;
     const SchemeFields f = split_scheme(scheme);
     if (f.dev <= OCT_DEV_DT) return 1.0;
-    const double D = (double)(1u << f.log2D), w = f.dev == OCT_DEV_CDB ? 1.0 : 5.0;
+    const double D = (double)(1u << f.log2D), w = f.dev == OCT_DEV_CDB ? 1.0 : 5.0;   // DB and DBh: 5
     return ((D - w) / D) * ((D - w) / D);   // Eq. (9) :137 with reading R9
 }
 

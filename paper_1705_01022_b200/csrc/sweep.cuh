@@ -24,7 +24,7 @@
 namespace octb {
 
 enum : int { kBlkSync = 0, kBlkDelayed = 1, kBlkDT = 2 };
-enum : uint32_t { kDevDTr = 0, kDevDT = 1, kDevDB = 2, kDevCDB = 3 };
+enum : uint32_t { kDevDTr = 0, kDevDT = 1, kDevDB = 2, kDevCDB = 3, kDevDBh = 4 };
 
 struct SweepParams {
     uint32_t* lat;                  // packed lattice, (L/4)^2 words
@@ -32,7 +32,7 @@ struct SweepParams {
     uint32_t L;
     uint32_t log2L;
     uint32_t t;                     // absolute MCS index of this sweep
-    uint32_t si;                    // position of this launch in the set permutation (0..3); 0 for DB/cDB
+    uint32_t si;                    // position of this launch in the set permutation (0..3); DBh: interval 0/1; else 0
     uint32_t P16, Q16;              // acceptance thresholds, accept iff r16 < P16 (R18)
     uint32_t dev;                   // device-layer scheme
     uint32_t ndom;                  // domains in this launch
@@ -152,8 +152,11 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     if (dom >= P.ndom) return;                       // whole group leaves together (own barrier id)
 
     // ---- a1: per-MCS control from the global stream (:144, :150; R10) --------------------------
+    // DB with t_async = 1/2 (kDevDBh, :204-206, R27): the launch is interval P.si of the sweep, with its own
+    // origin (global stream c0 = interval), half of the collective steps, streams keyed by set = interval
+    const bool half = P.dev == kDevDBh;
     uint32_t Gw[4];
-    philox4x32_10(0u, 0u, kTagGlobal << 30, t, P.rk, Gw);
+    philox4x32_10(half ? P.si : 0u, 0u, kTagGlobal << 30, t, P.rk, Gw);
     uint32_t gx, gy, set, dead_w;
     if (P.dev <= kDevDT) {
         const uint32_t Ox = P.dev == kDevDTr ? (Gw[0] & Lm) : 0u, Oy = P.dev == kDevDTr ? (Gw[1] & Lm) : 0u;
@@ -166,7 +169,7 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     } else {
         uint32_t Ox = Gw[0] & Lm, Oy = Gw[1] & Lm;
         if (P.dev == kDevCDB) { Ox &= ~3u; Oy &= ~3u; }                 // :166 coarse grid
-        set = 0u;
+        set = half ? P.si : 0u;
         const uint32_t lnt = P.log2L - LOG2D;
         const uint32_t I = dom & ((1u << lnt) - 1u), J = dom >> lnt;
         gx = (Ox + (I << LOG2D)) & Lm;
@@ -198,8 +201,10 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     int net = 0, d00 = 0;
     const uint32_t dead_lim = (uint32_t)D - dead_w;
 
+    const uint32_t k4_begin = half ? P.si * (uint32_t)(SH::NSTEP / 8) : 0u;
+    const uint32_t k4_end = half ? k4_begin + (uint32_t)(SH::NSTEP / 8) : (uint32_t)(SH::NSTEP / 4);
 #pragma unroll 1
-    for (uint32_t k4 = 0; k4 < (uint32_t)(SH::NSTEP / 4); ++k4) {
+    for (uint32_t k4 = k4_begin; k4 < k4_end; ++k4) {
         uint32_t rw[CPT][4];
 #pragma unroll
         for (int j = 0; j < CPT; ++j) philox4x32_10(k4, tg + j * G, c2c, t, P.rk, rw[j]);

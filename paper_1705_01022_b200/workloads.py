@@ -16,7 +16,7 @@ from dataclasses import dataclass
 import numpy as np
 
 # ---- public scheme code (include/oct.h): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 -------------
-DEV_DTR, DEV_DT, DEV_DB, DEV_CDB = 0, 1, 2, 3
+DEV_DTR, DEV_DT, DEV_DB, DEV_CDB, DEV_DBH = 0, 1, 2, 3, 4
 BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR = 0, 1, 2, 3
 INIT_FLAT, INIT_FLAT_SHIFTED, INIT_FROM_DEVICE = 0, 1, 2
 
@@ -27,7 +27,7 @@ def scheme_code(dev: int, blk: int, log2D: int, tcx: int = 1, tcy: int = 1) -> i
 
 def scheme_name(code: int) -> str:
     dev, blk = code & 15, (code >> 4) & 15
-    return (["DTr", "DT", "DB", "cDB"][dev] + ["DB", "DBd", "DT", "DTr"][blk]
+    return (["DTr", "DT", "DB", "cDB", "DBh"][dev] + ["DB", "DBd", "DT", "DTr"][blk]
             + f",TC={(code >> 8) & 15},{(code >> 12) & 15},D={1 << ((code >> 16) & 31)}")
 
 

@@ -43,7 +43,8 @@ def test_scheme_checks_match_the_header():
         assert ok(128, code)
     assert not ok(128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7))            # L < 2D
     assert not ok(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6, 0, 0))      # DT needs TC >= 1,1 (:182)
-    assert not ok(256, wl.scheme_code(4, 0, 6)) and not ok(256, wl.scheme_code(0, 4, 6))
+    assert not ok(256, wl.scheme_code(5, 0, 6)) and not ok(256, wl.scheme_code(0, 4, 6))
+    assert ok(256, wl.scheme_code(wl.DEV_DBH, wl.BLK_DB, 6))
     assert ok(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 6)) and not ok(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 6, 0, 1))
     assert not ok(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 4))            # D=16 not built
     assert not ok(100, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5))

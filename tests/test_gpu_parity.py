@@ -53,6 +53,9 @@ SMALL = [
     (256, wl.scheme_code(wl.DEV_DT, wl.BLK_DT, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DT, 6), 0.6, 0.4, 8),
+    (256, wl.scheme_code(wl.DEV_DBH, wl.BLK_DB, 6), 1.0, 0.0, 8),               # DB with t_async = 1/2
+    (256, wl.scheme_code(wl.DEV_DBH, wl.BLK_DT, 6), 0.7, 0.3, 4),
+    (512, wl.scheme_code(wl.DEV_DBH, wl.BLK_DB, 8), 0.9, 0.1, 3),
     (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DT, 6), 1.0, 0.0, 8),
     (64, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5), 1.0, 0.0, 16),               # L = 2D: a single tile
