@@ -131,3 +131,50 @@ def test_config4_L131072_sampled_boxes():
     replay_boxes(L, seed, code, log2D, p, q, pre, 6, h00, net, post, [(99991, 70001), (L - 300, L - 400)])
     check_invariants(sim, post)
     sim.close()
+
+
+def test_config2_L4096_mixed_rates_late_time_boxes():
+    """BASELINE config 3 (L = 4096, p = 0.9, q = 0.1, seed 7, DTrDB with delayed borders, D = 128) deep into the
+    run: MCS 1000 -> 1001 and 4999 -> 5000 replayed by the oracle on boxes (the first 2 MCS are compared in full
+    in test_gpu_parity.py); mean height and W^2 sums stay consistent with the counters all the way."""
+    cfg = wl.CONFIGS[2]
+    L, seed, code = cfg.L, cfg.seeds[0], cfg.scheme
+    log2D = (code >> 16) & 31
+    sim = binding.Sim(L, seed)
+    t_now = 0
+    for t in (1000, cfg.n_mcs - 1):
+        sim.oct_sweep(t - t_now, cfg.p, cfg.q, code)
+        pre = sim.oct_export()
+        h00, net = sim.oct_counters()
+        sim.oct_sweep(1, cfg.p, cfg.q, code)
+        t_now = t + 1
+        post = sim.oct_export()
+        replay_boxes(L, seed, code, log2D, cfg.p, cfg.q, pre, t, h00, net, post, [(777, 1234), (L - 900, L - 650)])
+        S1, S2, c, net2 = check_invariants(sim, post)
+        assert net2 > net                                         # p > q: the surface keeps growing
+    assert sim.oct_mcs() == cfg.n_mcs
+    sim.close()
+
+
+def test_config1_L1024_every_scheme_at_the_end_of_the_run():
+    """BASELINE config 2 (L = 1024, p = 1, q = 0, 2000 MCS, D = 128): for every device-layer x block-layer scheme
+    the paper defines, the last MCS of the run (1999 -> 2000) replayed by the oracle on the WHOLE lattice from the
+    GPU's exported pre-state (the first MCS are compared in test_gpu_parity.py)."""
+    cfg = wl.CONFIGS[1]
+    L, seed = cfg.L, 1
+    schemes = list(wl.ALL_SCHEMES(7)) + [wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 7), wl.scheme_code(wl.DEV_DBH, wl.BLK_DB, 7),
+                                         wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 2, 2), wl.scheme_code(wl.DEV_DTR, wl.BLK_DB_DELAYED, 7)]
+    orc = Oracle(L, seed)
+    for code in schemes:
+        sim = binding.Sim(L, seed)
+        sim.oct_sweep(cfg.n_mcs - 1, cfg.p, cfg.q, code)
+        pre = sim.oct_export()
+        h00, net = sim.oct_counters()
+        sim.oct_sweep(1, cfg.p, cfg.q, code)
+        orc.set_lattice(pre, h00=h00, net=net, t=cfg.n_mcs - 1)
+        orc.sweep(1, cfg.p, cfg.q, code)
+        assert (sim.oct_export() == orc.lattice).all(), wl.scheme_name(code)
+        assert sim.oct_counters() == (orc.h00, orc.net), wl.scheme_name(code)
+        assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == orc.sums(), wl.scheme_name(code)
+        sim.close()
+    orc.close()
