@@ -40,7 +40,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if res.returncode:
             raise RuntimeError("nvcc failed:\n" + res.stderr[-4000:])
         with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
-            f.write(res.stderr)
+            # registers / spills / shared memory per kernel; compile times would change on every build
+            f.write("".join(l for l in res.stderr.splitlines(True) if "Compile time" not in l))
         os.replace(tmp, LIB)
     return LIB
 
