@@ -15,25 +15,9 @@ from __future__ import annotations
 import argparse
 import json
 import math
-import sys
 import time
 
 from . import binding, workloads as wl
-
-
-def _strip(argv, flags):
-    """argv without the given `--flag value` pairs"""
-    out, skip = [], False
-    for a in argv:
-        if skip:
-            skip = False
-        elif a in flags:
-            skip = True
-        elif any(a.startswith(f + "=") for f in flags):
-            pass
-        else:
-            out.append(a)
-    return out
 
 
 def log_grid(t_max: int, per_decade: int, t_min: int = 1):
@@ -88,7 +72,7 @@ def main(argv=None):
     ap.add_argument("--p", type=float, default=1.0)
     ap.add_argument("--q", type=float, default=0.0)
     ap.add_argument("--seed", type=int, default=1)
-    ap.add_argument("--seeds", type=int, default=1, help="ensemble: run seeds seed .. seed+seeds-1 one after the other and average")
+    ap.add_argument("--seeds", type=int, default=1, help="ensemble: run seeds seed .. seed+seeds-1 concurrently (one stream each) and average")
     ap.add_argument("--log2D", type=int, default=6)
     ap.add_argument("--tcx", type=int, default=1)
     ap.add_argument("--tcy", type=int, default=1)
@@ -97,69 +81,81 @@ def main(argv=None):
     ap.add_argument("--per-decade", type=int, default=8)
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
-    if args.seeds > 1:
-        runs = []
-        for sd in range(args.seed, args.seed + args.seeds):
-            sub = list(argv if argv is not None else sys.argv[1:])
-            one = main(_strip(sub, ("--seeds", "--seed", "--out")) + ["--seed", str(sd)])
-            runs.append(one["rows"])
-        ens = ensemble_mean(runs)
-        for r in ens:
-            print("ensemble " + " ".join(f"{k}={v:.6g}" if isinstance(v, float) else f"{k}={v}" for k, v in r.items()))
-        if args.out:
-            with open(args.out, "w") as f:
-                json.dump({"seeds": list(range(args.seed, args.seed + args.seeds)), "ensemble": ens}, f, indent=1)
-        return {"ensemble": ens}
 
     import torch
     L, N = args.L, args.L * args.L
     code = wl.scheme_code(args.dev, args.blk, args.log2D, args.tcx, args.tcy)
-    sim = binding.Sim(L, args.seed)
     grid = log_grid(args.mcs, args.per_decade)
     if args.snap:
         grid = sorted(set(grid) | {args.snap} | {args.snap + t for t in log_grid(args.mcs - args.snap, args.per_decade) if args.snap + t <= args.mcs})
-    w2_dev = torch.empty(4, dtype=torch.int64, device=sim.device)
-    ch_dev = torch.empty(5, dtype=torch.int64, device=sim.device)
-    cs_dev = torch.empty(6, dtype=torch.int64, device=sim.device)
-    snap = anchor = None
-    rows, t_now = [], 0
+
+    # one simulation per seed, each on its own stream: small lattices do not fill the GPU alone, so the
+    # members of an ensemble run concurrently (they share nothing; every call only enqueues work)
+    seeds = list(range(args.seed, args.seed + args.seeds))
+    runs = []
+    for sd in seeds:
+        stream = torch.cuda.Stream() if len(seeds) > 1 else torch.cuda.current_stream()
+        with torch.cuda.stream(stream):
+            sim = binding.Sim(L, sd)
+        runs.append({"seed": sd, "sim": sim, "stream": stream, "snap": None, "anchor": None, "rows": [],
+                     "w2": torch.empty(4, dtype=torch.int64, device=sim.device),
+                     "ch": torch.empty(5, dtype=torch.int64, device=sim.device),
+                     "cs": torch.empty(6, dtype=torch.int64, device=sim.device)})
     torch.cuda.synchronize()
     wall0 = time.perf_counter()
+    t_now = 0
     for t in grid:
-        sim.oct_sweep(t - t_now, args.p, args.q, code)
+        for r in runs:                                           # enqueue on every member's stream ...
+            sim, st = r["sim"], r["stream"]
+            sim.oct_sweep(t - t_now, args.p, args.q, code, stream=st)
+            sim.oct_width2(r["w2"], stream=st)
+            if args.snap and t == args.snap:
+                with torch.cuda.stream(st):
+                    r["snap"], r["anchor"] = sim.oct_snapshot(stream=st)
+            if r["snap"] is not None:
+                sim.oct_autocorr(r["snap"], r["anchor"], r["ch"], stream=st)
+                sim.oct_slope_autocorr(r["snap"], r["cs"], stream=st)
         t_now = t
-        sim.oct_width2(w2_dev)
-        if args.snap and t == args.snap:
-            snap, anchor = sim.oct_snapshot()
-        S1, S2, c, net = (int(v) for v in w2_dev.cpu())
-        row = {"t": t, "w2": binding.oct_w2_from_sums(L, S1, S2), "mean_h": c + S1 / N, "net": net}
-        if snap is not None:
-            sim.oct_autocorr(snap, anchor, ch_dev)
-            sim.oct_slope_autocorr(snap, cs_dev)
-            St, Ss, Sts, _, _ = (int(v) for v in ch_dev.cpu())
-            xx, yy, xt, yt, xs, ys = (int(v) for v in cs_dev.cpu())
-            row["c_h"] = binding.oct_c_from_sums(L, St, Ss, Sts)
-            row["c_s"] = binding.oct_cs_from_sums(2 * N, xx + yy, xt + yt, xs + ys)
-        rows.append(row)
-    torch.cuda.synchronize()
+        torch.cuda.synchronize()                                 # ... then read the integer sums back
+        for r in runs:
+            S1, S2, c, net = (int(v) for v in r["w2"].cpu())
+            row = {"t": t, "w2": binding.oct_w2_from_sums(L, S1, S2), "mean_h": c + S1 / N, "net": net}
+            if r["snap"] is not None:
+                St, Ss, Sts, _, _ = (int(v) for v in r["ch"].cpu())
+                xx, yy, xt, yt, xs, ys = (int(v) for v in r["cs"].cpu())
+                row["c_h"] = binding.oct_c_from_sums(L, St, Ss, Sts)
+                row["c_s"] = binding.oct_cs_from_sums(2 * N, xx + yy, xt + yt, xs + ys)
+            r["rows"].append(row)
     wall = time.perf_counter() - wall0
 
-    prev = None
-    for r in rows:                                               # Eq. (8): effective exponents between grid points
-        if prev is not None:
-            r["beta_eff"] = (eff_exponent(r["w2"], r["t"], prev["w2"], prev["t"]) or 0.0) / 2 if r["t"] > 1 else None
-            if "c_h" in r and "c_h" in prev and args.snap and prev["t"] > args.snap:
-                r["lambda_h_over_z_eff"] = -(eff_exponent(r["c_h"], r["t"] / args.snap, prev["c_h"], prev["t"] / args.snap) or float("nan"))
-        prev = r
-    result = {"L": L, "p": args.p, "q": args.q, "seed": args.seed, "scheme": wl.scheme_name(code), "mcs": args.mcs,
-              "snap": args.snap, "wall_s": wall, "attempts_per_s_incl_observables": args.mcs * N / wall, "rows": rows}
-    for r in rows:
-        print(" ".join(f"{k}={v:.6g}" if isinstance(v, float) else f"{k}={v}" for k, v in r.items()))
-    print(f"# {wl.scheme_name(code)} L={L}: {args.mcs} MCS in {wall:.1f} s = {args.mcs * N / wall:.4g} attempts/s including the observables")
+    for r in runs:
+        prev = None
+        for row in r["rows"]:                                    # Eq. (8): effective exponents between grid points
+            if prev is not None:
+                row["beta_eff"] = (eff_exponent(row["w2"], row["t"], prev["w2"], prev["t"]) or 0.0) / 2 if row["t"] > 1 else None
+                if "c_h" in row and "c_h" in prev and args.snap and prev["t"] > args.snap:
+                    row["lambda_h_over_z_eff"] = -(eff_exponent(row["c_h"], row["t"] / args.snap, prev["c_h"], prev["t"] / args.snap) or float("nan"))
+            prev = row
+        r["sim"].close()
+
+    fmt = lambda d: " ".join(f"{k}={v:.6g}" if isinstance(v, float) else f"{k}={v}" for k, v in d.items())
+    total = len(seeds) * args.mcs * N
+    result = {"L": L, "p": args.p, "q": args.q, "seeds": seeds, "scheme": wl.scheme_name(code), "mcs": args.mcs, "snap": args.snap,
+              "wall_s": wall, "attempts_per_s_incl_observables": total / wall}
+    if len(seeds) == 1:
+        result["seed"] = seeds[0]
+        result["rows"] = runs[0]["rows"]
+        for row in result["rows"]:
+            print(fmt(row))
+    else:
+        result["runs"] = [{"seed": r["seed"], "rows": r["rows"]} for r in runs]
+        result["ensemble"] = ensemble_mean([r["rows"] for r in runs])
+        for row in result["ensemble"]:
+            print("ensemble " + fmt(row))
+    print(f"# {wl.scheme_name(code)} L={L}: {len(seeds)} x {args.mcs} MCS in {wall:.1f} s = {total / wall:.4g} attempts/s including the observables")
     if args.out:
         with open(args.out, "w") as f:
             json.dump(result, f, indent=1)
-    sim.close()
     return result
 
 

@@ -32,4 +32,3 @@ def test_ensemble_mean_and_standard_error():
     assert e[1]["w2"] == 5.0 and e[1]["mean_h_sem"] == pytest.approx(1.0)
     assert e[1]["beta_eff"] == pytest.approx(math.log(5.0 / 2.0) / math.log(10.0) / 2)
     assert "c_h" not in e[0]
-    assert run._strip(["--L", "64", "--seeds", "3", "--seed=2", "--out", "x"], ("--seeds", "--seed", "--out")) == ["--L", "64"]
