@@ -137,7 +137,7 @@ const char* oct_last_error(const oct_ctx*);             /* text of the last CUDA
 
 /* Implementation options.  They never change results (every kernel is bit-identical to the oracle), only
  * which kernel runs.  OCT_OPT_KERNEL: AUTO picks the link-entry kernel (one 32-bit entry of four link
- * bytes per site in shared memory, no atomics) for DTr/DT with D <= 128 and the bit-packed kernel
+ * bytes per site in shared memory, no atomics) for D <= 128 (>= 32 cells per domain) and the bit-packed kernel
  * otherwise; BITPACKED forces the latter; LINKS_B selects the alternative work split (another number of
  * warps per domain) where one is built.  EINVAL for unknown options / values. */
 enum { OCT_OPT_KERNEL = 1 };

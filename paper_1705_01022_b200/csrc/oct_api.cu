@@ -109,10 +109,11 @@ bool find_launch(int ld, int tx, int ty, int blk, SweepLaunch* out)
 
 // ---- link-entry sweep kernel (sweep_links.cuh): DTr/DT device layer, D <= 128 ------------------------
 template <int LD, int TX, int TY, int BLK, int W, int DPB>
-SweepLaunch make_links_launch()
+SweepLaunch make_links_launch(bool dead)
 {
     using SH = LinkShape<LD, TX, TY, W, DPB>;
-    return SweepLaunch{sweep_links_kernel<LD, TX, TY, BLK, W, DPB>, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
+    return SweepLaunch{dead ? sweep_links_kernel<LD, TX, TY, BLK, W, DPB, true> : sweep_links_kernel<LD, TX, TY, BLK, W, DPB, false>,
+                       SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
 }
 
 // (log2 D, tcx, tcy, warps per domain, domains per CTA): variant A is the default (the faster one on
@@ -123,14 +124,14 @@ SweepLaunch make_links_launch()
     X(7, 0, 0, 8, 1) X(7, 1, 1, 8, 1) X(7, 2, 2, 2, 1) X(7, 2, 1, 4, 1) X(7, 3, 2, 1, 1) X(7, 4, 1, 1, 1)
 #define OCT_LINK_SHAPES_B(X) X(6, 1, 1, 2, 2) X(7, 1, 1, 4, 1)
 
-bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, SweepLaunch* out)
+bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out)
 {
 #define X(LD, TX, TY, W, DPB)                                                                        \
     if (ld == LD && tx == TX && ty == TY) {                                                          \
-        if (blk == kBlkSync) { *out = make_links_launch<LD, TX, TY, kBlkSync, W, DPB>(); return true; }       \
-        if (blk == kBlkDelayed) { *out = make_links_launch<LD, TX, TY, kBlkDelayed, W, DPB>(); return true; } \
+        if (blk == kBlkSync) { *out = make_links_launch<LD, TX, TY, kBlkSync, W, DPB>(dead); return true; }       \
+        if (blk == kBlkDelayed) { *out = make_links_launch<LD, TX, TY, kBlkDelayed, W, DPB>(dead); return true; } \
         if constexpr (TX >= 1 && TY >= 1) {                                                          \
-            if (blk == kBlkDT) { *out = make_links_launch<LD, TX, TY, kBlkDT, W, DPB>(); return true; }       \
+            if (blk == kBlkDT) { *out = make_links_launch<LD, TX, TY, kBlkDT, W, DPB>(dead); return true; }       \
         }                                                                                            \
         return false;                                                                                \
     }
@@ -265,10 +266,11 @@ int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* 
     const int blk = (f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR) ? kBlkDT
                   : (f.blk == OCT_BLK_DB_DELAYED || (P16 > 0 && Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
     SweepLaunch sl;
-    // the link-entry kernel serves the tiled device layers on domains that fit shared memory unpacked;
-    // the bit-packed kernel serves everything else (D = 256, dead-border device layers, tiny domains)
-    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED && f.dev <= OCT_DEV_DT &&
-                       find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B, &sl);
+    // the link-entry kernel serves domains that fit shared memory unpacked; the bit-packed kernel serves
+    // everything else (D = 256, domains with fewer than 32 cells)
+    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED &&
+                       find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B,
+                                         f.dev > OCT_DEV_DT, &sl);
     if (!links && !find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &sl)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (sl.smem > 48 * 1024)

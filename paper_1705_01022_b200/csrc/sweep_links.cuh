@@ -1,6 +1,6 @@
-// Sweep kernel, link-entry layout: one launch = one domain-set sweep of the DTr / DT device-layer
-// schemes of arXiv 1705.01022 (Sec. 3.0.2-3.0.3) with any of the single-hit block
-// layers (Sec. 3.1, :168-174), for device-layer domains of D <= 128 sites.
+// Sweep kernel, link-entry layout: one launch = one domain-set sweep of any device-layer scheme of
+// arXiv 1705.01022 (DTr / DT: Sec. 3.0.2-3.0.3; DB / cDB / DBh: Sec. 3.0.1, :133-140, :166)
+// with any of the single-hit block layers (Sec. 3.1, :168-174), for device-layer domains of D <= 128 sites.
 //
 // Why a second layout (profiles/r1_a_*.md): on the bit-packed window the update test costs ~115 SASS
 // instructions per attempt, almost all of them shift/mask arithmetic and shared-memory atomics, and the
@@ -160,9 +160,11 @@ struct Rule {
 };
 
 // The collective single-hit steps of one domain sweep (:168-174).
-template <class SH, int BLK, bool ONEDIR, bool ALWAYS>
+// DEAD: dead-border device layer (:135): attempts whose domain-local x or y is >= dead_lim are not carried out.
+template <class SH, int BLK, bool ONEDIR, bool ALWAYS, bool DEAD>
 __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint32_t* __restrict__ BT, uint32_t tg, int grp,
-                                         uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16, uint32_t dtr_mask)
+                                         uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16, uint32_t dtr_mask,
+                                         uint32_t dead_lim, uint32_t k4_begin, uint32_t k4_end)
 {
     constexpr int CX = SH::CX, CY = SH::CY, G = SH::G, CPT = SH::CPT;
     constexpr uint32_t LOG2NCX = 0 + (SH::NCX == 1 ? 0 : SH::NCX == 2 ? 1 : SH::NCX == 4 ? 2 : SH::NCX == 8 ? 3 : SH::NCX == 16 ? 4 : 5);
@@ -179,8 +181,18 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
     }
     const Rule<ONEDIR, ALWAYS> rule(P16, Q16);
 
+    // decision for the site packed in v (x | y << 8 before wrapping); idx receives its entry index
+    auto decide_site = [&](uint32_t v, uint32_t w, uint32_t& idx) -> int {
+        idx = site_index<SH>(v);
+        if constexpr (DEAD) {
+            const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
+            if ((vm & 0xFFu) >= dead_lim || (vm >> 8) >= dead_lim) return 0;      // dead border: not carried out
+        }
+        return rule.decide(Sb[idx], w);
+    };
+
 #pragma unroll 1
-    for (uint32_t k4 = 0; k4 < (uint32_t)(SH::NSTEP / 4); ++k4) {
+    for (uint32_t k4 = k4_begin; k4 < k4_end; ++k4) {
         uint32_t rw[CPT][4];
 #pragma unroll
         for (int j = 0; j < CPT; ++j) philox4x32_10(k4, tg + j * G, c2c, t, rk, rw[j]);
@@ -199,9 +211,7 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
-                    const uint32_t v = (w & FM) + cellc[j] + sc;
-                    idx[j] = site_index<SH>(v);
-                    dec[j] = rule.decide(Sb[idx[j]], w);
+                    dec[j] = decide_site((w & FM) + cellc[j] + sc, w, idx[j]);
                 }
                 group_sync<SH::WPD, SH::DPB>(grp);
 #pragma unroll
@@ -210,19 +220,18 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
             } else if constexpr (BLK == kBlkDelayed) {
                 // delayed borders (:174): bulk, then edges, then corners (R15)
                 const uint32_t sc = Bw & FM;
-                uint32_t cls[CPT];
+                uint32_t cls[CPT], vv[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t f = rw[j][kk] & FM;
-                    const uint32_t v = f + cellc[j] + sc;
-                    idx[j] = site_index<SH>(v);
+                    vv[j] = f + cellc[j] + sc;
                     cls[j] = (uint32_t)((f & 0xFFu) == (uint32_t)(CX - 1)) + (uint32_t)((f >> 8) == (uint32_t)(CY - 1));
                 }
 #pragma unroll
                 for (uint32_t phase = 0; phase < 3; ++phase) {
                     int dec[CPT];                    // cells of one phase never touch common links (R15): loads first
 #pragma unroll
-                    for (int j = 0; j < CPT; ++j) dec[j] = cls[j] == phase ? rule.decide(Sb[idx[j]], rw[j][kk]) : 0;
+                    for (int j = 0; j < CPT; ++j) dec[j] = cls[j] == phase ? decide_site(vv[j], rw[j][kk], idx[j]) : 0;
 #pragma unroll
                     for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
                     group_sync<SH::WPD, SH::DPB>(grp);
@@ -237,8 +246,7 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, const uint3
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
-                    idx[j] = site_index<SH>((w & FM) + cellc[j] + qc);
-                    dec[j] = rule.decide(Sb[idx[j]], w);
+                    dec[j] = decide_site((w & FM) + cellc[j] + qc, w, idx[j]);
                 }
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
@@ -258,7 +266,10 @@ __device__ __forceinline__ int row_links_up(const uint32_t* Sb, uint32_t x00, ui
     return n;
 }
 
-template <int LOG2D, int TCX, int TCY, int BLK, int WPD, int DPB>
+// DEAD = false: tiled device layers DTr / DT (four launches per MCS, one per domain set);
+// DEAD = true : dead-border device layers DB / cDB / DBh (all tiles in one launch; the rim of width dead_w is
+//               never updated, and words shared with the next tile are neither counted nor written, :166).
+template <int LOG2D, int TCX, int TCY, int BLK, int WPD, int DPB, bool DEAD>
 __global__ void __launch_bounds__(LinkShape<LOG2D, TCX, TCY, WPD, DPB>::NTHREADS)
 sweep_links_kernel(const __grid_constant__ SweepParams P)
 {
@@ -277,17 +288,35 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
     if (dom >= P.ndom) return;                       // whole group leaves together (own barrier id)
 
     // ---- a1: per-MCS control from the global stream (:144, :150; R10) --------------------------
+    const bool half = DEAD && P.dev == kDevDBh;      // DB with t_async = 1/2: this launch is interval P.si (R27)
     uint32_t Gw[4];
-    philox4x32_10(0u, 0u, kTagGlobal << 30, t, P.rk, Gw);
-    const uint32_t Ox = P.dev == kDevDTr ? (Gw[0] & Lm) : 0u, Oy = P.dev == kDevDTr ? (Gw[1] & Lm) : 0u;
-    const uint32_t set = lex_perm4_at(Gw[2] % 24u, P.si);
-    const uint32_t lnt = P.log2L - LOG2D - 1u;                          // log2 tiles per edge
-    const uint32_t I = dom & ((1u << lnt) - 1u), J = dom >> lnt;
-    const uint32_t gx = (Ox + (I << (LOG2D + 1)) + ((set & 1u) << LOG2D)) & Lm;
-    const uint32_t gy = (Oy + (J << (LOG2D + 1)) + ((set >> 1) << LOG2D)) & Lm;
+    philox4x32_10(half ? P.si : 0u, 0u, kTagGlobal << 30, t, P.rk, Gw);
+    uint32_t gx, gy, set, dead_w;
+    if constexpr (!DEAD) {
+        const uint32_t Ox = P.dev == kDevDTr ? (Gw[0] & Lm) : 0u, Oy = P.dev == kDevDTr ? (Gw[1] & Lm) : 0u;
+        set = lex_perm4_at(Gw[2] % 24u, P.si);
+        const uint32_t lnt = P.log2L - LOG2D - 1u;                      // log2 tiles per edge
+        const uint32_t I = dom & ((1u << lnt) - 1u), J = dom >> lnt;
+        gx = (Ox + (I << (LOG2D + 1)) + ((set & 1u) << LOG2D)) & Lm;
+        gy = (Oy + (J << (LOG2D + 1)) + ((set >> 1) << LOG2D)) & Lm;
+        dead_w = 0u;
+    } else {
+        uint32_t Ox = Gw[0] & Lm, Oy = Gw[1] & Lm;
+        if (P.dev == kDevCDB) { Ox &= ~3u; Oy &= ~3u; }                 // :166 coarse grid
+        set = half ? P.si : 0u;
+        const uint32_t lnt = P.log2L - LOG2D;
+        const uint32_t I = dom & ((1u << lnt) - 1u), J = dom >> lnt;
+        gx = (Ox + (I << LOG2D)) & Lm;
+        gy = (Oy + (J << LOG2D)) & Lm;
+        dead_w = P.dev == kDevCDB ? 1u : 5u;                            // :166, R22
+    }
     const uint32_t offx = gx & 3u, offy = gy & 3u;
     const uint32_t LW = L >> 2, LWm = LW - 1u, wx0 = gx >> 2, wy0 = gy >> 2;
     uint32_t* Sb = S + offy * SH::P + offx;          // entry of the domain's site (0,0)
+    // window words this domain counts and writes back: all of them, or (dead border) only those that hold no
+    // site of the next tile -- the last active site's E / N links still lie inside them (:166)
+    const uint32_t ncol = DEAD ? ((offx + (uint32_t)D - dead_w) >> 2) + 1u : (uint32_t)NW;
+    const uint32_t nrow = DEAD ? ((offy + (uint32_t)D - dead_w) >> 2) + 1u : (uint32_t)NW;
 
     // ---- a2: stage-in (:164): packed words -> link entries -------------------------------------
     int net = 0;                                     // deposits - removals, from the x-moments (see x_moment)
@@ -310,7 +339,7 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
             if (idx < (uint32_t)(NW * NW)) {
                 const uint32_t jw = idx / NW, iw = idx - jw * NW;
                 expand_word<SH>(S, iw, jw, A[it], Ew[it], Nw[it]);
-                net += x_moment(A[it], iw);
+                if (!DEAD || (iw < ncol && jw < nrow)) net += x_moment(A[it], iw);
             }
         }
     }
@@ -336,14 +365,21 @@ sweep_links_kernel(const __grid_constant__ SweepParams P)
     // launch-uniform specialisation of the acceptance rule (the sync variant is only used with p*q = 0, R16)
     const bool onedir = BLK == kBlkSync || P.P16 == 0u || P.Q16 == 0u;
     const uint32_t T16 = P.Q16 == 0u ? P.P16 : P.Q16;
-    if (onedir && T16 == 65536u) run_steps<SH, BLK, true, true>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask);
-    else if (onedir)             run_steps<SH, BLK, true, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask);
-    else if constexpr (BLK != kBlkSync) run_steps<SH, BLK, false, false>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask);
+    const uint32_t dead_lim = (uint32_t)D - dead_w;
+    const uint32_t k4_begin = half ? P.si * (uint32_t)(SH::NSTEP / 8) : 0u;
+    const uint32_t k4_end = half ? k4_begin + (uint32_t)(SH::NSTEP / 8) : (uint32_t)(SH::NSTEP / 4);
+#define OCT_RUN(ONEDIR, ALWAYS) \
+    run_steps<SH, BLK, ONEDIR, ALWAYS, DEAD>(Sb, BT, tg, grp, c2c, t, P.rk, P.P16, P.Q16, P.dtr_mask, dead_lim, k4_begin, k4_end)
+    if (onedir && T16 == 65536u) OCT_RUN(true, true);
+    else if (onedir)             OCT_RUN(true, false);
+    else if constexpr (BLK != kBlkSync) OCT_RUN(false, false);
+#undef OCT_RUN
     // every variant of run_steps ends with a group barrier: the entries are final here
 
     // ---- a7: stage-out (:164): whole packed words of the window ---------------------------------
     for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
         const uint32_t jw = idx / NW, iw = idx - jw * NW;
+        if (DEAD && !(iw < ncol && jw < nrow)) continue;
         const uint32_t word = gather_word<SH>(S, iw, jw);
         P.lat[(size_t)((wy0 + jw) & LWm) * LW + ((wx0 + iw) & LWm)] = word;
         net -= x_moment(word, iw);
