@@ -16,6 +16,8 @@ namespace octb {
 // sigma_y(0, 4wy+j) is bit 8j+1 of word (wx=0, wy).
 constexpr int kAnchorThreads = 1024;
 
+constexpr int kAnchorMaxPer = 32;      // L <= 2^17: at most 2^15 words in column 0 = 32 per thread
+
 __global__ void __launch_bounds__(kAnchorThreads)
 column_anchor_kernel(const uint32_t* __restrict__ lat, uint32_t L, int32_t* __restrict__ anchor)
 {
@@ -23,31 +25,42 @@ column_anchor_kernel(const uint32_t* __restrict__ lat, uint32_t L, int32_t* __re
     const uint32_t LW = L >> 2;
     const uint32_t per = (LW + kAnchorThreads - 1) / kAnchorThreads;     // words of column 0 per thread
     const uint32_t w0 = threadIdx.x * per;
-    int32_t sum = 0;
-    for (uint32_t w = w0; w < w0 + per && w < LW; ++w) {
-        const uint32_t v = lat[(size_t)w * LW];
-        sum += 2 * __popc(v & 0x02020202u) - 4;
+    // the column is strided by one lattice row per word (one sector each): issue all of this thread's loads at
+    // once and keep the words in registers for the second pass
+    uint32_t v[kAnchorMaxPer];
+#pragma unroll
+    for (int k = 0; k < kAnchorMaxPer; ++k) {
+        const uint32_t w = w0 + k;
+        v[k] = ((uint32_t)k < per && w < LW) ? lat[(size_t)w * LW] : 0u;
     }
+    int32_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < kAnchorMaxPer; ++k)
+        if ((uint32_t)k < per && w0 + k < LW) sum += 2 * __popc(v[k] & 0x02020202u) - 4;
     part[threadIdx.x] = sum;
     __syncthreads();
     // inclusive Hillis-Steele scan over the per-thread totals
     for (int off = 1; off < kAnchorThreads; off <<= 1) {
-        int32_t v = threadIdx.x >= (unsigned)off ? part[threadIdx.x - off] : 0;
+        int32_t u = threadIdx.x >= (unsigned)off ? part[threadIdx.x - off] : 0;
         __syncthreads();
-        part[threadIdx.x] += v;
+        part[threadIdx.x] += u;
         __syncthreads();
     }
-    // h(0, 4*w0 - 1 + 1 ...) : running value entering this thread's first word.  The scan counts
-    // sigma_y(0,0) as well, which closes the loop around the torus and is not part of the path from
-    // (0,0); remove it.
+    // running value entering this thread's first word.  The scan counts sigma_y(0,0) as well, which closes the
+    // loop around the torus and is not part of the path from (0,0); remove it.
     const int32_t s00 = (lat[0] >> 1) & 1u ? 1 : -1;
     int32_t run = part[threadIdx.x] - sum - s00;
-    for (uint32_t w = w0; w < w0 + per && w < LW; ++w) {
-        const uint32_t v = lat[(size_t)w * LW];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            run += (v >> (8 * j + 1)) & 1u ? 1 : -1;
-            anchor[4 * w + j] = run;
+    for (int k = 0; k < kAnchorMaxPer; ++k) {
+        const uint32_t w = w0 + k;
+        if ((uint32_t)k < per && w < LW) {
+            int32_t a[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                run += (v[k] >> (8 * j + 1)) & 1u ? 1 : -1;
+                a[j] = run;
+            }
+            *reinterpret_cast<int4*>(anchor + 4 * w) = make_int4(a[0], a[1], a[2], a[3]);
         }
     }
 }
