@@ -38,3 +38,18 @@ def test_cdb_leaves_a_pattern_dtr_does_not_and_wide_borders_add_noise():
     assert cdb_mean > 2e-4 and cdb_mean > 2.5 * cdb_sem and cdb_mean > 4 * abs(dtr_mean)   # finite plateau
     assert abs(db_mean) < 3 * db_sem                                            # no persistent correlation ...
     assert db_sem > 2.5 * dtr_sem                                               # ... but clearly more noise
+
+
+def test_finer_block_layer_decomposition_gives_a_smaller_roughness_prefactor():
+    """a finer DD samples the lattice more evenly, which lowers the noise amplitude and with it the
+    prefactor of W^2(t) -- TC=1,1 lies below TC=2,2 (and both grow with the same exponent).  L = 4096, 8 seeds."""
+    def w2_at(tc, t_probe=(32, 100, 316)):
+        out = run.main(["--L", "4096", "--mcs", "316", "--log2D", "7", "--tcx", str(tc), "--tcy", str(tc),
+                        "--seeds", "8", "--per-decade", "4"])
+        rows = {r["t"]: r for r in out["ensemble"]}
+        return [(rows[t]["w2"], rows[t]["w2_sem"]) for t in t_probe]
+    fine, coarse = w2_at(1), w2_at(2)
+    for k, ((wf, sf), (wc, sc)) in enumerate(zip(fine, coarse)):
+        assert wf < wc and (wc - wf) / wc < 0.03                        # below, by a percent-level correction only
+        if k < 2:                                                       # early times: far outside the sampling noise
+            assert (wc - wf) > 3 * math.hypot(sf, sc)
