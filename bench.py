@@ -243,13 +243,13 @@ def main():
     attempts_per_launch = L * L / 4
     achieved = I_ALG * attempts_per_launch / launch_s / 1e12                     # T lane-instr/s
     peak = N_SM * SMSP * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "sweep_traffic.json")
+    traffic = None                                   # dram bytes per sweep launch from the committed ncu capture
+    tp = os.path.join(ROOT, "profiles", "sweep_traffic.csv")
     if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get(f"L{L}_D{1 << args.log2D}")
-        except Exception:
-            traffic = None
+        for line in open(tp):
+            c = line.strip().split(",")
+            if c[0] == f"L{L}_D{1 << args.log2D}" and args.kernel != 1 and args.blk == 0:
+                traffic = int(c[1])
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-instr/s", "frac": achieved / peak,
                 "traffic": traffic, "kernel": "sweep_links_kernel" if (args.log2D <= 7 and args.kernel != 1) else "sweep_kernel", "avg_launch_ms": launch_s * 1e3, "instr_per_attempt": I_ALG,
                 "peak_src": f"148 SM x 4 SMSP x 32 lanes x sm_max_mhz ({peaks['src']})",
