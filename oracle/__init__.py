@@ -80,6 +80,7 @@ def lib():
         L.orc_heights.argtypes = [vp, vp]; L.orc_heights.restype = None
         L.orc_heights_rowpath.argtypes = [vp, vp]; L.orc_heights_rowpath.restype = None
         L.orc_sums.argtypes = [vp, vp]; L.orc_sums.restype = i32
+        L.orc_sums_rowpath.argtypes = [vp, vp]; L.orc_sums_rowpath.restype = i32
         L.orc_autocorr_sums.argtypes = [vp, vp, vp]; L.orc_autocorr_sums.restype = i32
         L.orc_slope_autocorr_sums.argtypes = [vp, vp, vp]; L.orc_slope_autocorr_sums.restype = i32
         _lib = L
@@ -220,10 +221,11 @@ class Oracle:
         (self._l.orc_heights_rowpath if rowpath else self._l.orc_heights)(self._h, out.ctypes.data)
         return out
 
-    def sums(self):
-        """(S1, S2, c, net) with c = h(0,0)."""
+    def sums(self, rowpath: bool = False):
+        """(S1, S2, c, net) with c = h(0,0).  rowpath: integrate up column 0 and along the rows, streaming (no
+        height array; the only form that fits in memory at L = 2^17)."""
         o = np.zeros(4, dtype=np.int64)
-        rc = self._l.orc_sums(self._h, o.ctypes.data)
+        rc = (self._l.orc_sums_rowpath if rowpath else self._l.orc_sums)(self._h, o.ctypes.data)
         if rc:
             raise MemoryError
         return tuple(int(v) for v in o)

@@ -512,6 +512,26 @@ int orc_sums(const orc_state *s, int64_t out[4])
     return 0;
 }
 
+/* The same four numbers as orc_sums along the OTHER integration path (up column 0, then along each row, as in
+ * orc_heights_rowpath) without materialising the heights: O(1) extra memory, so it also serves L = 2^17, where the
+ * int32 height array would take 64 GiB.  Pinned against orc_sums (tests/test_oracle_rule.py). */
+int orc_sums_rowpath(const orc_state *s, int64_t out[4])
+{
+    const uint32_t L = s->L;
+    int64_t S1 = 0, S2 = 0, col = 0;                    /* col = h(0,y) - c */
+    for (uint32_t y = 0; y < L; ++y) {
+        if (y > 0) col += get_sy(s, 0, y) ? 1 : -1;
+        int64_t d = col;
+        S1 += d; S2 += d * d;
+        for (uint32_t x = 1; x < L; ++x) {
+            d += get_sx(s, x, y) ? 1 : -1;
+            S1 += d; S2 += d * d;
+        }
+    }
+    out[0] = S1; out[1] = S2; out[2] = s->h00; out[3] = s->net;
+    return 0;
+}
+
 /* out = {S_t, S_s, S_ts, c_t, c_s}: C_h(t,s) = S_ts/N - (S_t/N)(S_s/N)   (Eq. (6) :92, reading R7) */
 int orc_autocorr_sums(const orc_state *now, const orc_state *snap, int64_t out[5])
 {

@@ -1,4 +1,7 @@
-"""Build liboct_b200.so (the C-ABI product library) in-tree with nvcc for sm_100a."""
+"""Build liboct_b200.so (the C-ABI product library) in-tree with nvcc for sm_100a.
+
+    python -m paper_1705_01022_b200.build [ptxas_report.txt]
+"""
 from __future__ import annotations
 
 import os
@@ -29,7 +32,8 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, ptxas_info: str | None = None) -> str:
+    """ptxas_info: optional path that receives ptxas' per-kernel register / spill / shared-memory report."""
     if force or stale():
         tmp = LIB + f".tmp{os.getpid()}"
         cmd = [nvcc(), *NVCC_FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
@@ -39,12 +43,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
             print(res.stderr)
         if res.returncode:
             raise RuntimeError("nvcc failed:\n" + res.stderr[-4000:])
-        with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
-            # registers / spills / shared memory per kernel; compile times would change on every build
-            f.write("".join(l for l in res.stderr.splitlines(True) if "Compile time" not in l))
+        if ptxas_info:
+            with open(ptxas_info, "w") as f:
+                f.write("".join(l for l in res.stderr.splitlines(True) if "Compile time" not in l))
         os.replace(tmp, LIB)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose=False))
+    import sys
+    print(build(force=True, verbose=False, ptxas_info=sys.argv[1] if len(sys.argv) > 1 else None))

@@ -1,10 +1,10 @@
 """Seeded synthetic workloads shared by the tests, the bench, the oracle side and the CUDA side.
 
 This module holds NONE of the method's arithmetic (no update rule, no RNG of the method, no domain
-decomposition): only (a) the parameter sets of the five BASELINE.json configs, (b) the bit layout of
-the public `scheme` code and of the canonical packed lattice (both are the boundary's data format,
-include/oct.h), and (c) a generator of arbitrary valid slope fields that is unrelated to the dynamics
-(used to feed the height-reconstruction and reduction kernels, and to pin the oracle's heights).
+decomposition): only (a) the parameter sets of the five BASELINE.json configs and (b) the bit layout of
+the public `scheme` code (the boundary's data format, include/oct.h).  The generator of arbitrary valid
+surfaces that feeds the reconstruction / reduction kernels and pins the oracle's heights is test
+infrastructure and lives in tests/helpers/surfaces.py.
 
 The paper uses no dataset: its workloads are square periodic power-of-two lattices started flat and
 driven with p=1, q=0, so the configs below *are* the paper's workload shape.
@@ -12,8 +12,6 @@ driven with p=1, q=0, so the configs below *are* the p
 from __future__ import annotations
 
 from dataclasses import dataclass
-
-import numpy as np
 
 # ---- public scheme code (include/oct.h): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 -------------
 DEV_DTR, DEV_DT, DEV_DB, DEV_CDB, DEV_DBH = 0, 1, 2, 3, 4
@@ -58,45 +56,6 @@ CONFIGS = (
 # with the recommended DB block layer
 ALL_SCHEMES = lambda lD: tuple(scheme_code(d, b, lD) for d in (DEV_DTR, DEV_DT, DEV_DB, DEV_CDB)  # noqa: E731
                                for b in (BLK_DB, BLK_DT))
-
-
-# ---- canonical packed format (include/oct.h; "each 32-bit word encodes 4x4 sites") ----
-def pack_slopes(sx: np.ndarray, sy: np.ndarray) -> np.ndarray:
-    """sx, sy: (L, L) arrays indexed [y, x] of 0/1 bits (1 <=> slope +1 towards the site from its
-    west / south neighbour).  Returns (L/4, L/4) uint32 words: site (4wx+i, 4wy+j) has sigma_x at bit
-    2(4j+i) and sigma_y at bit 2(4j+i)+1 of word [wy, wx]."""
-    L = sx.shape[0]
-    assert sx.shape == (L, L) and sy.shape == (L, L) and L % 4 == 0
-    n = L // 4
-    out = np.zeros((n, n), dtype=np.uint32)
-    for j in range(4):
-        for i in range(4):
-            b = 2 * (4 * j + i)
-            out |= (sx[j::4, i::4].astype(np.uint32) & 1) << np.uint32(b)
-            out |= (sy[j::4, i::4].astype(np.uint32) & 1) << np.uint32(b + 1)
-    return out
-
-
-def pack_heights(h: np.ndarray) -> np.ndarray:
-    """Canonical words of a periodic height field h[y, x] whose neighbours differ by exactly 1."""
-    dx = h - np.roll(h, 1, axis=1)
-    dy = h - np.roll(h, 1, axis=0)
-    assert (np.abs(dx) == 1).all() and (np.abs(dy) == 1).all(), "not a valid octahedron surface"
-    return pack_slopes((dx == 1), (dy == 1))
-
-
-def _balanced_walk(rng: np.random.Generator, L: int) -> np.ndarray:
-    steps = np.array([1] * (L // 2) + [-1] * (L // 2), dtype=np.int32)
-    rng.shuffle(steps)
-    return np.cumsum(steps).astype(np.int32) - steps[0]        # w[0] = 0, |w[i+1]-w[i]| = 1, periodic
-
-
-def separable_surface(L: int, seed: int, offset: int = 0) -> np.ndarray:
-    """A valid periodic surface unrelated to the dynamics: h[y, x] = a[x] + b[y] + offset with a, b
-    closed +-1 walks.  h[0, 0] = offset.  Rough (|h| ~ sqrt(L)), so it exercises carries and signs."""
-    rng = np.random.default_rng(seed)
-    a, b = _balanced_walk(rng, L), _balanced_walk(rng, L)
-    return (a[None, :] + b[:, None] + offset).astype(np.int32)
 
 
 def rank_seed(base_seed: int, rank: int) -> int:

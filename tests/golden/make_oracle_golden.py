@@ -4,7 +4,15 @@ a handful of small runs.  Calls ONLY oracle/ (never the CUDA path).  The file is
 arithmetic (a later change to it must be deliberate: regenerate and say why in the commit) and lets GPU tests compare
 against stored oracle results without re-running the oracle.
 
-    python tests/golden/make_oracle_golden.py            # rewrite the file
+    python tests/golden/make_oracle_golden.py            # rewrite oracle_runs.txt (seconds)
+    python tests/golden/make_oracle_golden.py --full c4_D64     # one FULL-SIZE run -> full_c4_D64.txt (minutes to hours)
+    python tests/golden/make_oracle_golden.py --full all        # every full-size run, one after the other
+
+Full-size runs (BASELINE.json configs 3, 4 and 5 as `north_star` states them: "bit-exact lattice vs oracle" for the whole
+5000-MCS mixed-rate run at L = 4096, "the oracle checked bit-exact on the first 2 MCS" at L = 2^16, the first MCS at
+L = 2^17; PAPER.md:262 gives L = 2^16, :232 L = 2^17, :174 the p, q > 0 path).  One file per run so that they can be
+produced in parallel; tests/test_gpu_fullsize.py hashes oct_export() at the same checkpoints.  At these sizes the sums
+are taken along the row path without a height array (Oracle.sums(rowpath=True), pinned against the plain form).
 """
 import hashlib
 import os
@@ -29,6 +37,44 @@ RUNS = (
 )
 
 
+# name -> (L, seed, p, q, scheme, checkpoints, every_mcs_sums)
+FULL_RUNS = {
+    # BASELINE config 4: L = 2^16, p = 1, q = 0, seed 1, DTrDB -- first 2 MCS, whole lattice
+    "c4_D64": (1 << 16, 1, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 6), (1, 2), False),
+    "c4_D128": (1 << 16, 1, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 7), (1, 2), False),
+    "c4_D256": (1 << 16, 1, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 8), (1, 2), False),
+    "c4_D64_TC22": (1 << 16, 1, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 6, 2, 2), (1, 2), False),   # PAPER.md:236-244 (Fig. 5)
+    # BASELINE config 5: L = 2^17 -- first MCS, whole lattice
+    "c5_D64": (1 << 17, 1, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 6), (1,), False),
+    # BASELINE config 3: L = 4096, p = 0.9, q = 0.1, seed 7, DTrDB (delayed borders), the whole 5000-MCS run:
+    # lattice hash every 500 MCS, and the sums after EVERY MCS hashed per 500-MCS window
+    "c3_D128": (4096, 7, 0.9, 0.1, scheme(DEV_DTR, BLK_DB, 7), tuple(range(500, 5001, 500)), True),
+}
+
+
+def full_lines(name):
+    L, seed, p, q, code, cps, every = FULL_RUNS[name]
+    yield "# name L seed p q scheme t sha256(lattice words, little endian) S1 S2 h00 net"
+    yield "# sums_sha name t0 t1 sha256(text 'S1 S2 h00 net\\n' for every MCS t0 < t <= t1)"
+    yield f"# written by `python tests/golden/make_oracle_golden.py --full {name}` from oracle/oct_oracle.c only"
+    o = Oracle(L, seed)
+    t_prev = 0
+    for t in cps:
+        if every:
+            hs = hashlib.sha256()
+            while o.t < t:
+                o.sweep(1, p, q, code)
+                hs.update(("%d %d %d %d\n" % o.sums(rowpath=True)).encode())
+            yield f"sums_sha {name} {t_prev} {t} {hs.hexdigest()}"
+        else:
+            o.sweep(t - o.t, p, q, code)
+        digest = hashlib.sha256(o.lattice.astype("<u4").tobytes()).hexdigest()
+        S1, S2, c, net = o.sums(rowpath=True)
+        yield f"{name} {L} {seed} {p} {q} {code} {t} {digest} {S1} {S2} {c} {net}"
+        t_prev = t
+    o.close()
+
+
 def lines():
     yield "# name L seed p q scheme t sha256(lattice words, little endian) S1 S2 h00 net"
     yield "# written by tests/golden/make_oracle_golden.py from oracle/oct_oracle.c only"
@@ -43,7 +89,18 @@ def lines():
 
 
 if __name__ == "__main__":
-    out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_runs.txt")
-    with open(out, "w") as f:
-        f.write("\n".join(lines()) + "\n")
-    print(out)
+    here = os.path.dirname(os.path.abspath(__file__))
+    if len(sys.argv) >= 3 and sys.argv[1] == "--full":
+        for name in (FULL_RUNS if sys.argv[2] == "all" else sys.argv[2:]):
+            out = os.path.join(here, f"full_{name}.txt")
+            with open(out + ".part", "w") as f:
+                for line in full_lines(name):
+                    f.write(line + "\n")
+                    f.flush()
+            os.replace(out + ".part", out)
+            print(out)
+    else:
+        out = os.path.join(here, "oracle_runs.txt")
+        with open(out, "w") as f:
+            f.write("\n".join(lines()) + "\n")
+        print(out)

@@ -52,3 +52,23 @@ def test_gpu_reproduces_the_golden_runs():
                 assert sha(sim.oct_export()) == digest, (name, t, kernel)
                 assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == sums, (name, t, kernel)
             sim.close()
+
+
+def test_full_size_golden_files_are_complete():
+    """The full-size oracle results (make_oracle_golden.py --full) that tests/test_gpu_fullsize.py compares with: every
+    run is present with all its checkpoints, and config 4's two domain sizes differ (the hashes pin a scheme, not a size)."""
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    want = {"c4_D64": [1, 2], "c4_D128": [1, 2], "c4_D256": [1, 2], "c4_D64_TC22": [1, 2], "c5_D64": [1],
+            "c3_D128": list(range(500, 5001, 500))}
+    seen = {}
+    for name, ts in want.items():
+        rows = [l.split() for l in open(os.path.join(here, f"full_{name}.txt")) if l.strip() and not l.startswith("#")]
+        cps = [r for r in rows if r[0] == name]
+        assert [int(r[6]) for r in cps] == ts, name
+        for r in cps:
+            L, S1, net = int(r[1]), int(r[8]), int(r[11])
+            assert len(r[7]) == 64 and S1 + L * L * int(r[10]) == L * L // 2 + 2 * net, (name, r[6])   # sum of heights
+            seen[(name, r[6])] = r[7]
+        if name == "c3_D128":
+            assert len([r for r in rows if r[0] == "sums_sha"]) == len(ts)
+    assert len(set(seen.values())) == len(seen)

@@ -9,6 +9,9 @@ replays that MCS on sampled boxes (one of them across the periodic seam, one aro
 site), and the packed words inside the boxes must be identical.  Properties that hold at any size cover
 the rest: slope conservation per row / column, the height-sum identity, C_h(s,s) sums == W^2 sums.
 """
+import hashlib
+import os
+
 import numpy as np
 import pytest
 
@@ -178,3 +181,71 @@ def test_config1_L1024_every_scheme_at_the_end_of_the_run():
         assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == orc.sums(), wl.scheme_name(code)
         sim.close()
     orc.close()
+
+
+# ---- whole-lattice parity at full size against stored oracle results --------------------------------------------
+# tests/golden/full_<name>.txt are written by `python tests/golden/make_oracle_golden.py --full <name>` from oracle/ only
+# (SHA-256 of the oracle's packed lattice + its integer sums at each checkpoint).  The CUDA path must reproduce them:
+# BASELINE config 4 "the oracle checked bit-exact on the first 2 MCS" (L = 2^16), config 5 first MCS
+# (L = 2^17, :232), config 3 the whole 5000-MCS mixed-rate run (p, q > 0: delayed borders, :174).
+GOLDEN_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def read_full(name):
+    cps, windows = [], {}
+    for line in open(os.path.join(GOLDEN_DIR, f"full_{name}.txt")):
+        f = line.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] == "sums_sha":
+            windows[int(f[3])] = (int(f[2]), f[4])
+        else:
+            assert f[0] == name
+            cps.append({"L": int(f[1]), "seed": int(f[2]), "p": float(f[3]), "q": float(f[4]), "code": int(f[5]), "t": int(f[6]),
+                        "sha": f[7], "sums": tuple(int(v) for v in f[8:12])})
+    return cps, windows
+
+
+def sha_words(words):
+    return hashlib.sha256(np.ascontiguousarray(words).astype("<u4", copy=False).tobytes()).hexdigest()
+
+
+@pytest.mark.parametrize("name,kernel", [("c4_D64", binding.OCT_KERNEL_AUTO), ("c4_D64", binding.OCT_KERNEL_BITPACKED),
+                                         ("c4_D128", binding.OCT_KERNEL_AUTO), ("c4_D256", binding.OCT_KERNEL_AUTO),
+                                         ("c4_D64_TC22", binding.OCT_KERNEL_AUTO), ("c5_D64", binding.OCT_KERNEL_AUTO)])
+def test_whole_lattice_equals_the_oracle_at_full_size(name, kernel):
+    cps, _ = read_full(name)
+    c0 = cps[0]
+    sim = binding.Sim(c0["L"], c0["seed"])
+    sim.oct_set_option(binding.OCT_OPT_KERNEL, kernel)
+    host = np.empty((c0["L"] // 4, c0["L"] // 4), dtype=np.uint32)
+    for c in cps:
+        sim.oct_sweep(c["t"] - sim.oct_mcs(), c["p"], c["q"], c["code"])
+        assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == c["sums"], (name, c["t"])
+        assert sim.oct_counters() == c["sums"][2:], (name, c["t"])
+        assert sha_words(sim.oct_export(host)) == c["sha"], (name, c["t"])
+    sim.close()
+
+
+def test_config3_whole_run_equals_the_oracle():
+    """BASELINE config 3 in full: L = 4096, p = 0.9, q = 0.1, seed 7, DTrDB D = 128 (delayed borders), 5000 MCS: the
+    lattice hash every 500 MCS and (S1, S2, h00, net) after EVERY MCS (W^2(t) and the mean height per MCS)."""
+    cps, windows = read_full("c3_D128")
+    assert [c["t"] for c in cps] == list(range(500, 5001, 500)) and len(windows) == len(cps)
+    c0 = cps[0]
+    sim = binding.Sim(c0["L"], c0["seed"])
+    out = torch.empty(4, dtype=torch.int64, device=sim.device)
+    for c in cps:
+        t0, want = windows[c["t"]]
+        assert t0 == sim.oct_mcs()
+        hs, rows = hashlib.sha256(), []
+        for _ in range(c["t"] - t0):
+            sim.oct_sweep(1, c["p"], c["q"], c["code"])
+            sim.oct_width2(out)
+            rows.append(out.clone())                      # stay asynchronous; read the window back at its end
+        for r in torch.stack(rows).cpu().numpy():
+            hs.update(("%d %d %d %d\n" % tuple(int(v) for v in r)).encode())
+        assert hs.hexdigest() == want, ("sums of MCS", t0, c["t"])
+        assert tuple(int(v) for v in rows[-1].cpu().numpy()) == c["sums"], c["t"]
+        assert sha_words(sim.oct_export()) == c["sha"], c["t"]
+    sim.close()

@@ -9,6 +9,7 @@ import pytest
 
 import oracle
 from oracle import Oracle
+from helpers import surfaces as sf
 from paper_1705_01022_b200 import binding, workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -167,19 +168,19 @@ def test_flat_shifted_symmetry_on_gpu():
                                         (2048, 6, 77), (4096, 7, -40000)])
 def test_heights_and_sums_on_synthetic_surfaces(L, seed, off):
     """Reconstruction / reduction kernels on surfaces unrelated to the dynamics (rough, ragged L)."""
-    h = wl.separable_surface(L, seed, off)
-    words = wl.pack_heights(h)
+    h = sf.separable_surface(L, seed, off)
+    words = sf.pack_heights(h)
     sim = binding.Sim(L, 0, wl.INIT_FROM_DEVICE, lattice=torch.from_numpy(words.view(np.int32).reshape(-1)).cuda())
     sim.oct_set_state(0, off, 17)
     orc = Oracle(L, 0); orc.set_lattice(words, h00=off, net=17)
     assert (sim.oct_heights().cpu().numpy() == h).all()
     assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == orc.sums()
     # autocorrelation against a second, different surface
-    h2 = wl.separable_surface(L, seed + 100, off - 5)
-    snap = torch.from_numpy(wl.pack_heights(h2).view(np.int32).reshape(-1)).cuda()
+    h2 = sf.separable_surface(L, seed + 100, off - 5)
+    snap = torch.from_numpy(sf.pack_heights(h2).view(np.int32).reshape(-1)).cuda()
     anchor = torch.tensor([off - 5, 3], dtype=torch.int64, device="cuda")
     got = tuple(int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy())
-    orc2 = Oracle(L, 0); orc2.set_lattice(wl.pack_heights(h2), h00=off - 5, net=3)
+    orc2 = Oracle(L, 0); orc2.set_lattice(sf.pack_heights(h2), h00=off - 5, net=3)
     assert got == orc.autocorr_sums(orc2)
     # slope autocorrelation (PAPER.md:85-88) against the same second surface, and C_s(s,s) = 1/4
     cs = tuple(int(v) for v in sim.oct_slope_autocorr(snap).cpu().numpy())

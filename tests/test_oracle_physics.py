@@ -88,7 +88,7 @@ def test_slope_autocorrelation_pins():
     """C_s of PAPER.md:85-88 on the lattice-gas variables n = slope bit.  Pins that do not go through the
     oracle's own packing: slopes taken straight from height arrays; the equal-time value 1/4 (n^2 = n,
     <n> = 1/2 by the periodic closure); the complement -1/4; the flat state against its one-site shift."""
-    from paper_1705_01022_b200.workloads import separable_surface, pack_heights   # seeded input generator, no method arithmetic
+    from helpers.surfaces import separable_surface, pack_heights   # seeded input generator, no method arithmetic
     L = 64
     ha, hb = separable_surface(L, 11, 5), separable_surface(L, 12, -3)
     a, b = Oracle(L, 0), Oracle(L, 0)

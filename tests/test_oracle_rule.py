@@ -11,7 +11,7 @@ import pytest
 
 import oracle
 from oracle import BLK_DB, BLK_DB_DELAYED, BLK_DT, DEV_CDB, DEV_DB, DEV_DT, DEV_DTR, Oracle, scheme
-from paper_1705_01022_b200 import workloads as wl
+from helpers import surfaces as sf
 
 
 # ---- brute force on the 4x4 periodic lattice ------------------------------------------------------
@@ -65,7 +65,7 @@ def test_bruteforce_4x4_every_state_every_site(surfaces4):
     n_min = n_max = 0
     o = Oracle(4, 0)
     for h in surfaces4:
-        words = wl.pack_heights(h)
+        words = sf.pack_heights(h)
         for y in range(4):
             for x in range(4):
                 for (P16, Q16) in ((65536, 0), (0, 65536), (65536, 65536)):
@@ -81,7 +81,7 @@ def test_bruteforce_4x4_every_state_every_site(surfaces4):
                         want = -1
                     assert d == want
                     assert (o.heights() == exp).all()
-                    assert (o.lattice == wl.pack_heights(exp)).all()
+                    assert (o.lattice == sf.pack_heights(exp)).all()
                     assert o.net == want
                 n_min += is_min(h, y, x)
                 n_max += is_max(h, y, x)
@@ -102,7 +102,7 @@ def test_acceptance_threshold_is_strict_less_than(surfaces4):
     y, x = int(ys[0]), int(xs[0])
     o = Oracle(4, 0)
     P16 = oracle.prob16(0.9)
-    o.set_lattice(wl.pack_heights(h))
+    o.set_lattice(sf.pack_heights(h))
     assert o.attempt(x, y, P16, P16, 0) == 0          # r16 == P16 -> reject
     assert o.attempt(x, y, P16 - 1, P16, 0) == 1      # r16 <  P16 -> accept
     o.close()
@@ -111,7 +111,7 @@ def test_acceptance_threshold_is_strict_less_than(surfaces4):
 def test_h00_tracking_on_origin_updates(surfaces4):
     o = Oracle(4, 0)
     for h in surfaces4[:200]:
-        o.set_lattice(wl.pack_heights(h), h00=0)
+        o.set_lattice(sf.pack_heights(h), h00=0)
         d = o.attempt(0, 0, 0, 65536, 65536)
         assert o.h00 == 2 * d
         exp = h.copy()
@@ -128,7 +128,7 @@ def test_flat_state(L):
     yy, xx = np.mgrid[0:L, 0:L]
     h = ((xx + yy) & 1).astype(np.int32)
     assert (o.heights() == h).all() and (o.heights(rowpath=True) == h).all()
-    assert (o.lattice == wl.pack_heights(h)).all()
+    assert (o.lattice == sf.pack_heights(h)).all()
     assert o.w2() == 0.25 and o.mean_height() == 0.5
     S1, S2, c, net = o.sums()
     assert (S1, S2, c, net) == (L * L // 2, L * L // 2, 0, 0)
@@ -154,14 +154,15 @@ def test_flat_shifted_is_the_complement():
 # ---- heights from an independent generator -----------------------------------------------------------
 @pytest.mark.parametrize("L,seed,off", [(16, 1, 0), (64, 2, -7), (256, 3, 1000)])
 def test_heights_of_separable_surface(L, seed, off):
-    h = wl.separable_surface(L, seed, off)
+    h = sf.separable_surface(L, seed, off)
     o = Oracle(L, 0)
-    o.set_lattice(wl.pack_heights(h), h00=off)
+    o.set_lattice(sf.pack_heights(h), h00=off)
     assert (o.heights() == h).all()
     assert (o.heights(rowpath=True) == h).all()
     S1, S2, c, _ = o.sums()
     d = h.astype(np.int64) - off
     assert (S1, S2, c) == (int(d.sum()), int((d * d).sum()), off)
+    assert o.sums(rowpath=True) == o.sums()            # streaming form used at L = 2^16, 2^17 (no height array)
     assert float(o.w2()) == pytest.approx(float(np.var(h.astype(np.float64))), rel=1e-12)
     o.close()
 
@@ -190,7 +191,7 @@ def check_valid_surface(o: Oracle):
     assert (SX + np.roll(SY, 1, axis=1) == SY + np.roll(SX, 1, axis=0)).all()
     h = o.heights()
     assert (h == o.heights(rowpath=True)).all()
-    assert (o.lattice == wl.pack_heights(h)).all()
+    assert (o.lattice == sf.pack_heights(h)).all()
     return h
 
 
@@ -223,6 +224,8 @@ def test_invariants_and_tracked_heights(code, p, q):
         assert (h == o.tracked_heights).all()
         assert int(h.astype(np.int64).sum()) == L * L // 2 + 2 * o.net
         assert o.h00 == h[0, 0]
+        d = h.astype(np.int64) - o.h00
+        assert o.sums(rowpath=True) == o.sums() == (int(d.sum()), int((d * d).sum()), o.h00, o.net)
     o.close()
 
 
