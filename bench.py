@@ -6,9 +6,10 @@
 
 Metric (BASELINE.json): site-update attempts per second at L = 2^16, p = 1, q = 0, scheme DTrDB
 (PAPER.md:262, :276).  One *step* is one pass of the whole hot path on the resident lattice:
-`--mcs-per-step` MCS of oct_sweep (4 launches per MCS), then oct_width2 and oct_autocorr against the
-waiting-time snapshot.  attempts = mcs_per_step * L^2 per step (rejected attempts count, :270).
+`--mcs-per-step` MCS of oct_sweep (4 launches per MCS), then the W^2 and C_h sums against the waiting-time
+snapshot in one pass (oct_observe).  attempts = mcs_per_step * L^2 per step (rejected attempts count, :270).
 The lattice (1 GiB) is larger than L2 (126 MB), so no explicit L2 flush is needed between steps.
+The same run also measures L = 2^17 (`also`), the second size BASELINE.json's north_star names.
 N > 1 runs N independent replicas (different seeds, no data-path collective: "replicas only").
 """
 from __future__ import annotations
@@ -29,13 +30,16 @@ sys.path.insert(0, ROOT)
 METRIC = "site_update_attempts_per_s"
 UNIT = "attempts/s"
 
-# Algorithmic lane-instructions per update attempt of the DTrDB sweep in the link-entry design (DESIGN.md
-# section 6): Philox4x32-10 40/4 = 10, site select 5, entry load + compare 2, five stores of an accepted
-# update (issued warp-wide) 5, step loop/sync 1, staging (expand + gather + moments per site) 9.
-I_ALG = 32.0
 # the paper's DTrDB throughput at L = 2^16, p=1, q=0 on Kepler GPUs, per GPU
 PAPER_ATTEMPTS_PER_S = 9.0e9
 N_SM, SMSP, LANES = 148, 4, 32
+# Conflict-free minimum of shared-memory wavefronts per warp-attempt (32 update attempts) of the link-entry sweep
+# (DESIGN.md section 5.1): 1 entry load + 5 stores of an accepted update (issued whenever a lane of the warp accepts)
+# + staging 2 x (68 x 68 entries x 4 B / 128 B) per 128 warp-attempts of a 64 x 64 domain + 1/8 block-step load.
+WAVEFRONTS_MIN = 1.0 + 5.0 + 2.0 * (68 * 68 * 4 / 128.0) / 128.0 + 0.125
+# Algorithmic lane-instructions per attempt: Philox 40/4 = 10, site select 5, entry load +
+# compare 2, five stores 5, loop/sync 1, staging per site 9.  The executed count comes from the committed ncu capture.
+I_ALG = 32.0
 
 
 def measured_peaks():
@@ -45,6 +49,21 @@ def measured_peaks():
             d = json.load(f)
         return {"hbm_gbs": d.get("hbm_gbs", 6650.0), "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "src": "measured"}
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+def ncu_counters(kernel: str, L: int, log2D: int, tcx: int, tcy: int, blk: int):
+    """Per-launch counters of the sweep kernel from the committed ncu capture (profiles/sweep_counters.csv: one row per
+    captured configuration; the .md beside it names the command).  None if this configuration was not captured."""
+    path = os.path.join(ROOT, "profiles", "sweep_counters.csv")
+    if not os.path.exists(path):
+        return None
+    rows = [l.strip().split(",") for l in open(path) if l.strip() and not l.startswith("#")]
+    hdr = rows[0]
+    for r in rows[1:]:
+        d = dict(zip(hdr, r))
+        if (d["kernel"], int(d["L"]), int(d["log2D"]), int(d["tcx"]), int(d["tcy"]), int(d["blk"])) == (kernel, L, log2D, tcx, tcy, blk):
+            return {k: (float(v) if k not in ("kernel", "source") else v) for k, v in d.items()}
+    return None
 
 
 class ClockSampler:
@@ -96,15 +115,39 @@ class ClockSampler:
         return out
 
 
-def time_oracle(L: int, log2D: int, n_mcs: int, seed: int):
-    """The CPU oracle as it stands, single thread, on a bounded sample of the workload."""
+def scheme_label(args):
+    name = "DTrDT" if getattr(args, "blk", 0) == 2 else "DTrDB"
+    return f"{name},TC={args.tcx},{args.tcy},D={1 << args.log2D}"
+
+
+def baseline_config_no(L):
+    return {256: 1, 1024: 2, 4096: 3, 1 << 16: 4, 1 << 17: 5}.get(L)
+
+
+def workload_config(args, oracle_sample_L=None):
+    n = baseline_config_no(args.L)
+    tag = f"BASELINE config {n}" if n else "custom size"
+    cfg = {"workload": f"{tag}: octahedron model, L={args.L} periodic, flat start, p=1 q=0, {scheme_label(args)}",
+           "L": args.L, "p": 1.0, "q": 0.0, "scheme": scheme_label(args), "mcs_per_step": args.mcs_per_step,
+           "burn_in_mcs": args.burn_in, "l2": "inputs larger than L2 (lattice %d MiB)" % (args.L * args.L // 4 >> 20),
+           "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
+    if oracle_sample_L is not None:
+        cfg["timed_sample"] = f"the oracle is timed on an L={oracle_sample_L} sample of this workload (same scheme, p, q, domain size)"
+        cfg["sample_L"] = oracle_sample_L
+    return cfg
+
+
+def time_oracle(L: int, code_args, n_mcs: int, seed: int, burn: int = 1, rs: bool = False):
+    """The CPU oracle as it stands, single thread, on a bounded sample of the workload (attempts/s, seconds, sums)."""
     import oracle
-    code = oracle.scheme(oracle.DEV_DTR, oracle.BLK_DB, log2D)
+    log2D, tcx, tcy, blk = code_args
+    code = oracle.scheme(oracle.DEV_DTR, blk, log2D, tcx, tcy)
     o = oracle.Oracle(L, seed)
-    o.sweep(1, 1.0, 0.0, code)               # leave the exactly-flat state (acceptance 0.5 -> ~0.2)
+    run = (lambda n: o.sweep_rs(n, 1.0, 0.0)) if rs else (lambda n: o.sweep(n, 1.0, 0.0, code))
+    run(burn)                                # leave the exactly-flat state (acceptance 0.5 -> ~0.2)
     t0 = time.perf_counter()
-    o.sweep(n_mcs, 1.0, 0.0, code)
-    S = o.sums()
+    run(n_mcs)
+    S = o.sums(rowpath=True)
     dt = time.perf_counter() - t0
     o.close()
     return n_mcs * L * L / dt, dt, S
@@ -114,19 +157,20 @@ def run_reference(args, rank: int, world: int):
     if rank != 0:
         return
     Ls, n_mcs = args.ref_L, args.ref_mcs
+    ca = (min(args.log2D, 8), args.tcx, args.tcy, args.blk)
     vals, times = [], []
     for i in range(args.warmup + args.steps):
-        v, dt, _ = time_oracle(Ls, min(args.log2D, 8), n_mcs, args.seed + i)
+        v, dt, _ = time_oracle(Ls, ca, n_mcs, args.seed + i, burn=args.ref_burn)
         if i >= args.warmup:
             vals.append(v); times.append(dt)
     value = sum(vals) / len(vals)
-    sample = (f"per step: {n_mcs} MCS of DTrDB(D={1 << args.log2D}) incl. the W2 sums on an L={Ls} flat-start lattice "
+    sample = (f"per step: {n_mcs} MCS of {scheme_label(args)} incl. the W2 sums on an L={Ls} lattice after {args.ref_burn} burn-in MCS from flat "
               f"(same scheme, p, q and domain size as the L={args.L} workload; oracle/oct_oracle.c, gcc -O2, 1 thread)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-        "config": workload_config(args),
+        "config": workload_config(args, oracle_sample_L=Ls),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -134,12 +178,79 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(args):
-    name = "DTrDT" if getattr(args, "blk", 0) == 2 else "DTrDB"
-    return {"workload": f"c3_L{args.L}: octahedron model, L={args.L} periodic, flat start, p=1 q=0, {name} TC=1,1 D={1 << args.log2D}",
-            "L": args.L, "p": 1.0, "q": 0.0, "scheme": f"{name},TC=1,1,D={1 << args.log2D}", "mcs_per_step": args.mcs_per_step,
-            "burn_in_mcs": args.burn_in, "l2": "inputs larger than L2 (lattice %d MiB)" % (args.L * args.L // 4 >> 20),
-            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
+def measure(sim, code, M, steps, warmup, torch, dist, replicas, binding, snap, anchor, obs_out, sampler=None):
+    """warmup + `steps` timed steps of (M MCS of oct_sweep, then W^2 and C_h sums in one pass); CUDA events on the stream."""
+    stream = torch.cuda.current_stream()
+    what = binding.OCT_OBS_W2 | binding.OCT_OBS_CH
+
+    def step(ev=None):
+        if ev:
+            ev[0].record(stream)
+        sim.oct_sweep(M, 1.0, 0.0, code)
+        if ev:
+            ev[1].record(stream)
+        sim.oct_observe(what, snap, anchor, obs_out)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    if sampler is not None:
+        sampler.start()
+    n0 = sim.oct_launch_count()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(steps):
+        step(evs[i])
+    e1.record(stream)
+    barrier()
+    launches = sim.oct_launch_count() - n0
+    clocks = sampler.stop() if sampler is not None else None
+    total_ms = e0.elapsed_time(e1)
+    per_step_sweep = [a.elapsed_time(b) for a, b in evs]
+    total_ms, sweep_ms = replicas.max_over_ranks([total_ms, sum(per_step_sweep)], dist, sim.device)
+    return {"total_ms": total_ms, "sweep_ms": sweep_ms, "launches": launches, "clocks": clocks, "barrier": barrier,
+            "window_ms": per_step_sweep}
+
+
+def roofline_block(args, L, peaks, sweep_ms, total_ms, n_sweep_launches, kernel):
+    """Roofline of the dominant kernel (one domain-set sweep): shared-memory data pipe, with the issue-slot view beside it."""
+    launch_s = sweep_ms * 1e-3 / n_sweep_launches
+    attempts_per_launch = L * L / 4
+    warp_attempts = attempts_per_launch / 32
+    f_hz = peaks["sm_max_mhz"] * 1e6
+    peak_wf = N_SM * f_hz / 1e9                                    # G wavefronts/s: one per clock per SM
+    achieved = WAVEFRONTS_MIN * warp_attempts / launch_s / 1e9
+    cnt = ncu_counters(kernel, L, args.log2D, args.tcx, args.tcy, args.blk) or ncu_counters(kernel, 1 << 16, args.log2D, args.tcx, args.tcy, args.blk)
+    rf = {"bound": "smem", "achieved": achieved, "peak": peak_wf, "unit": "Gwavefront/s", "frac": achieved / peak_wf,
+          "traffic": None, "kernel": kernel, "avg_launch_ms": launch_s * 1e3, "attempts_per_launch": attempts_per_launch,
+          "wavefronts_per_warp_attempt_min": WAVEFRONTS_MIN,
+          "peak_src": f"148 SM x 1 shared-memory wavefront/clk x sm_max_mhz ({peaks['src']})",
+          "hbm_gbs_of_sweep": 0.5 * (1.0 + 4.0 / (1 << args.log2D)) ** 2 * attempts_per_launch / launch_s / 1e9,
+          "sweep_share_of_step": sweep_ms / total_ms}
+    peak_issue = N_SM * SMSP * LANES * f_hz / 1e12
+    issue = {"unit": "Tlane-instr/s", "peak": peak_issue, "instr_per_attempt_algorithmic": I_ALG,
+             "achieved_algorithmic": I_ALG * attempts_per_launch / launch_s / 1e12}
+    issue["frac_algorithmic"] = issue["achieved_algorithmic"] / peak_issue
+    if cnt is not None:
+        scale = attempts_per_launch / (cnt["L"] * cnt["L"] / 4)        # counters of an L = 2^16 capture scale with the domain count
+        rf["traffic"] = int(cnt["dram_bytes"] * scale)
+        wpa = cnt["wavefronts_shared"] / (cnt["L"] * cnt["L"] / 4 / 32)
+        rf["wavefronts_per_warp_attempt_measured"] = wpa
+        rf["pipe_utilisation"] = wpa * warp_attempts / launch_s / 1e9 / peak_wf
+        ipa = cnt["inst_executed"] / (cnt["L"] * cnt["L"] / 4 / 32)
+        issue["instr_per_attempt_executed"] = ipa
+        issue["achieved_executed"] = ipa * attempts_per_launch / launch_s / 1e12
+        issue["frac_executed"] = issue["achieved_executed"] / peak_issue
+        rf["counters_src"] = cnt["source"]
+    rf["issue_slots"] = issue
+    return rf
 
 
 def main():
@@ -150,13 +261,17 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=1 << 16)
     ap.add_argument("--log2D", type=int, default=6)
-    ap.add_argument("--mcs-per-step", type=int, default=8)
+    ap.add_argument("--mcs-per-step", type=int, default=32)
     ap.add_argument("--burn-in", type=int, default=32)
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--ref-L", type=int, default=4096, help="lattice edge of the oracle's timed sample")
-    ap.add_argument("--ref-mcs", type=int, default=32)
+    ap.add_argument("--ref-mcs", type=int, default=16)
+    ap.add_argument("--ref-burn", type=int, default=4)
+    ap.add_argument("--tcx", type=int, default=1, help="thread-cell size TC=tcx,tcy (log2 of the cell edge in 4-site words, PAPER.md:180)")
+    ap.add_argument("--tcy", type=int, default=1)
     ap.add_argument("--blk", type=int, default=0, help="block layer: 0 DB (the benched DTrDB), 2 DT (DTrDT, PAPER.md:268)")
     ap.add_argument("--kernel", type=int, default=0, help="OCT_OPT_KERNEL value: 0 auto, 1 bit-packed, 2 link-entry variant B")
+    ap.add_argument("--also-L", type=int, default=1 << 17, help="second lattice size measured in the same run (0: none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-heights", action="store_true", help="skip timing oct_heights (needs a 4*L*L byte buffer)")
@@ -171,9 +286,10 @@ def main():
         run_reference(args, rank, world)
         return
 
+    if rank == 0:                                # one rank builds (if stale) before the others load the library
+        from paper_1705_01022_b200 import binding
+        binding.load()
     import torch
-    from paper_1705_01022_b200 import binding, replicas, workloads as wl
-
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product has no CPU path (use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
@@ -181,80 +297,37 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    from paper_1705_01022_b200 import binding, replicas, workloads as wl
 
     L, M = args.L, args.mcs_per_step
-    code = wl.scheme_code(wl.DEV_DTR, args.blk, args.log2D)
+    code = wl.scheme_code(wl.DEV_DTR, args.blk, args.log2D, args.tcx, args.tcy)
     seed = replicas.replica_seed(args.seed, rank)
+    warm = max(args.warmup, 3)
+    peaks = measured_peaks()
+    kernel = "sweep_links_kernel" if (args.log2D <= 7 and args.kernel != 1) else "sweep_kernel"
+
     sim = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
     sim.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)
     stream = torch.cuda.current_stream()
-    sim.oct_sweep(args.burn_in, 1.0, 0.0, code)            # evolved state: acceptance ~0.17 (not the flat 0.5)
+    sim.oct_sweep(args.burn_in, 1.0, 0.0, code)            # evolved state: acceptance ~0.2 (not the flat 0.5)
     snap, anchor = sim.oct_snapshot()
-    w2_out = torch.empty(4, dtype=torch.int64, device=sim.device)
-    ac_out = torch.empty(5, dtype=torch.int64, device=sim.device)
-    cs_out = torch.empty(6, dtype=torch.int64, device=sim.device)
-
-    def step(ev=None):
-        if ev:
-            ev[0].record(stream)
-        sim.oct_sweep(M, 1.0, 0.0, code)
-        if ev:
-            ev[1].record(stream)
-        sim.oct_width2(w2_out)
-        sim.oct_autocorr(snap, anchor, ac_out)
-
-    def barrier():
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-    n0 = sim.oct_launch_count()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for i in range(args.steps):
-        step(evs[i])
-    e1.record(stream)
-    barrier()
-    launches = sim.oct_launch_count() - n0
-    clocks = sampler.stop() if rank == 0 else None
-    total_ms = e0.elapsed_time(e1)
-    sweep_ms = sum(a.elapsed_time(b) for a, b in evs)
-    total_ms, sweep_ms = replicas.max_over_ranks([total_ms, sweep_ms], dist, sim.device)
-    peaks = measured_peaks()
+    obs = torch.empty(16, dtype=torch.int64, device=sim.device)
+    m = measure(sim, code, M, args.steps, warm, torch, dist, replicas, binding, snap, anchor, obs,
+                sampler=ClockSampler(local_rank) if rank == 0 else None)
+    barrier = m["barrier"]
     attempts_per_step = M * L * L
-    value = replicas.aggregate_throughput(attempts_per_step, args.steps, world, total_ms)
+    value = replicas.aggregate_throughput(attempts_per_step, args.steps, world, m["total_ms"])
 
     # sanity of the state that was timed: sums are consistent with the counters
-    S = [int(v) for v in w2_out.cpu().numpy()]
+    S = [int(v) for v in obs.cpu().numpy()]
     h00, net = sim.oct_counters()
-    assert S[2] == h00 and S[3] == net and S[0] + L * L * h00 == L * L // 2 + 2 * net, "inconsistent state"
+    assert S[2] == h00 and S[3] == net and S[0] + L * L * h00 == L * L // 2 + 2 * net and S[4] == S[0], "inconsistent state"
 
-    # ---- roofline of the dominant kernel (sweep): issue-slot bound ---------------------------------
-    n_sweep_launches = args.steps * M * 4
-    launch_s = sweep_ms * 1e-3 / n_sweep_launches
-    attempts_per_launch = L * L / 4
-    achieved = I_ALG * attempts_per_launch / launch_s / 1e12                     # T lane-instr/s
-    peak = N_SM * SMSP * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
-    traffic = None                                   # dram bytes per sweep launch from the committed ncu capture
-    tp = os.path.join(ROOT, "profiles", "sweep_traffic.csv")
-    if os.path.exists(tp):
-        for line in open(tp):
-            c = line.strip().split(",")
-            if c[0] == f"L{L}_D{1 << args.log2D}" and args.kernel != 1 and args.blk == 0:
-                traffic = int(c[1])
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlane-instr/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": "sweep_links_kernel" if (args.log2D <= 7 and args.kernel != 1) else "sweep_kernel", "avg_launch_ms": launch_s * 1e3, "instr_per_attempt": I_ALG,
-                "peak_src": f"148 SM x 4 SMSP x 32 lanes x sm_max_mhz ({peaks['src']})",
-                "hbm_gbs_of_sweep": 0.5 * (1.0 + 4.0 / (1 << args.log2D)) ** 2 * attempts_per_launch / launch_s / 1e9,
-                "sweep_share_of_step": sweep_ms / total_ms}
+    roofline = roofline_block(args, L, peaks, m["sweep_ms"], m["total_ms"], args.steps * M * 4, kernel)
+    # sustained throughput: the sweep part of every timed step is a window of M MCS (PAPER.md:268 saw clocks drop after ~100 MCS)
+    win = sorted(L * L * M / (w * 1e-3) for w in m["window_ms"])
+    sustained = {"window_mcs": M, "windows": len(win), "median_attempts_per_s": win[len(win) // 2], "min": win[0], "max": win[-1]}
 
     # ---- observables (a8/a9): HBM-bound kernels, timed alone, algorithmic bytes / time -------------------
     def time_call(fn, reps=5):
@@ -267,10 +340,14 @@ def main():
         return a.elapsed_time(b) / reps
 
     lat_bytes = L * L // 4
+    w2_out = torch.empty(4, dtype=torch.int64, device=sim.device)
+    ac_out = torch.empty(5, dtype=torch.int64, device=sim.device)
+    cs_out = torch.empty(6, dtype=torch.int64, device=sim.device)
     observables = {}
     for name, fn, nbytes in (("oct_width2", lambda: sim.oct_width2(w2_out), lat_bytes),
                              ("oct_autocorr", lambda: sim.oct_autocorr(snap, anchor, ac_out), 2 * lat_bytes),
-                             ("oct_slope_autocorr", lambda: sim.oct_slope_autocorr(snap, cs_out), 2 * lat_bytes)):
+                             ("oct_slope_autocorr", lambda: sim.oct_slope_autocorr(snap, cs_out), 2 * lat_bytes),
+                             ("oct_observe(W2|CH|CS)", lambda: sim.oct_observe(7, snap, anchor, obs), 2 * lat_bytes)):
         ms = time_call(fn)
         observables[name] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm": nbytes / ms / 1e6 / peaks["hbm_gbs"]}
     if L <= (1 << 16) and not args.no_heights:
@@ -280,21 +357,21 @@ def main():
         observables["oct_heights"] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm": nbytes / ms / 1e6 / peaks["hbm_gbs"]}
         del hbuf
 
-    # ---- e2e: same step through the C ABI with HOST buffers ------------------------------------------
+    # ---- e2e: the same step through the C ABI with HOST buffers (pinned): the lattice goes up before and comes back
+    # after the sweeps, the sums come back through oct_fetch -----------------------------------------------
     e2e = None
     if not args.no_e2e:
         nb = binding.oct_lattice_bytes(L)
         host = torch.empty(nb // 4, dtype=torch.int32).pin_memory()
-        sums_host = torch.empty(9, dtype=torch.int64).pin_memory()
+        sums_host = torch.empty(16, dtype=torch.int64).pin_memory()
         sim.oct_export_to(host.data_ptr())
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
         def step_e2e():
-            sim.oct_upload(host.data_ptr())
+            sim.oct_upload(host.data_ptr())                          # the lattice exported by the previous step: counters stay valid
             sim.oct_sweep(M, 1.0, 0.0, code)
-            sim.oct_width2(w2_out)
-            sim.oct_autocorr(snap, anchor, ac_out)
-            sums_host[:4].copy_(w2_out, non_blocking=True)
-            sums_host[4:].copy_(ac_out, non_blocking=True)
+            sim.oct_observe(binding.OCT_OBS_W2 | binding.OCT_OBS_CH, snap, anchor, obs)
+            sim.oct_fetch(obs, sums_host.data_ptr(), 16 * 8)         # synchronises
             sim.oct_export_to(host.data_ptr())                       # synchronises
 
         ke = max(2, min(args.steps, 5))
@@ -306,30 +383,58 @@ def main():
             step_e2e()
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        wall = (time.perf_counter() - t0) * 1e3
-        ms = max(ms, wall)
+        ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3)
         ms = replicas.max_over_ranks([ms], dist, sim.device)[0]
+        assert int(sums_host[3]) == sim.oct_counters()[1]
         e2e = {"value": replicas.aggregate_throughput(attempts_per_step, ke, world, ms), "unit": UNIT, "h2d_bytes_per_step": nb,
-               "d2h_bytes_per_step": nb + 72, "steps": ke, "ms_per_step": ms / ke}
+               "d2h_bytes_per_step": nb + 128, "steps": ke, "ms_per_step": ms / ke}
+        del host
+    sim.close()
+    del snap, sim
 
-    # ---- the oracle timed on this box's host cores (rank 0, N = 1 only) -------------------------------
+    # ---- the second size north_star names (L = 2^17: 4 GiB packed), same scheme, in the same run ------------
+    also = None
+    if args.also_L and args.also_L != L and world == 1:
+        L2 = args.also_L
+        sim2 = binding.Sim(L2, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
+        sim2.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)
+        sim2.oct_sweep(args.burn_in, 1.0, 0.0, code)
+        snap2, anchor2 = sim2.oct_snapshot()
+        M2, K2 = max(1, M // 4), max(3, args.steps // 2)
+        m2 = measure(sim2, code, M2, K2, 3, torch, dist, replicas, binding, snap2, anchor2, obs)
+        v2 = M2 * L2 * L2 * K2 / (m2["total_ms"] * 1e-3)
+        a2 = argparse.Namespace(**vars(args)); a2.L = L2; a2.mcs_per_step = M2
+        also = {"config": workload_config(a2), "value": v2, "unit": UNIT, "steps": K2, "ms_per_step": m2["total_ms"] / K2,
+                "roofline": roofline_block(args, L2, peaks, m2["sweep_ms"], m2["total_ms"], K2 * M2 * 4, kernel)}
+        sim2.close()
+        del snap2, sim2
+
+    # ---- the oracle timed on this box's host cores (rank 0, N = 1 only): bounded samples ------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, dt, _ = time_oracle(args.ref_L, min(args.log2D, 8), args.ref_mcs, args.seed)
+        ca = (min(args.log2D, 8), args.tcx, args.tcy, args.blk)
+        v, dt, _ = time_oracle(args.ref_L, ca, args.ref_mcs, args.seed, burn=args.ref_burn)
+        v14, dt14, _ = time_oracle(1 << 14, ca, 2, args.seed, burn=1)
+        vrs, dtrs, _ = time_oracle(args.ref_L, ca, 4, args.seed, burn=1, rs=True)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"{args.ref_mcs} MCS of DTrDB(D={1 << args.log2D}) + W2 sums on an L={args.ref_L} flat-start lattice, "
-                         f"{dt:.1f} s, oracle/oct_oracle.c gcc -O2 single thread"}
+               "sample": f"{args.ref_mcs} MCS of {scheme_label(args)} + W2 sums on an L={args.ref_L} lattice ({args.ref_L * args.ref_L // 4 >> 20} MiB, cache-resident: "
+                         f"the oracle's most favourable case, cf. the paper's L=2^12 CPU figure, PAPER.md:270) after {args.ref_burn} burn-in MCS, "
+                         f"{dt:.1f} s, oracle/oct_oracle.c gcc -O2 single thread; the GPU figure is L={L} after {args.burn_in} burn-in MCS",
+               "others": [
+                   {"what": f"{scheme_label(args)}, L=16384 (64 MiB, out of cache), 2 MCS after 1", "value": v14, "seconds": dt14},
+                   {"what": f"true RS dynamics (PAPER.md:15/:44), L={args.ref_L}, 4 MCS after 1", "value": vrs, "seconds": dtrs}]}
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-                "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16) else None,
-                "dtype": "u32", "data": "synthetic", "config": workload_config(args), "clocks": clocks, "e2e": e2e,
-                "gpu_launches": launches, "roofline": roofline, "observables": observables, "cpu_baseline": cpu,
-                "paper_context": "PAPER.md:276 ~9e9 attempts/s on Kepler GPUs (other hardware; context, not a target)"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
+                "ms_per_step": m["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16 and args.blk == 0) else None,
+                "dtype": "u32", "data": "synthetic", "config": workload_config(args), "clocks": m["clocks"], "e2e": e2e,
+                "gpu_launches": m["launches"], "roofline": roofline, "sustained": sustained, "also": also,
+                "observables": observables, "cpu_baseline": cpu,
+                "vs_cpu_baseline": (value / world / cpu["value"]) if cpu else None,
+                "paper_context": "vs_baseline divides by PAPER.md:276's ~9e9 attempts/s (DTrDB, L=2^16, p=1, q=0) on Kepler GPUs: other hardware, "
+                                 "context, not a target; vs_cpu_baseline divides by the oracle timed in this run (cpu_baseline.sample says on what)"}
         print(json.dumps(line), flush=True)
-    sim.close()
     if dist is not None:
         dist.destroy_process_group()
 

@@ -13,6 +13,9 @@
  *    passed as void* (NULL = the legacy default stream).
  *  - Unless stated otherwise a call only ENQUEUES work on `stream` and returns; results land in
  *    device buffers in stream order.  Calls that touch host buffers say whether they synchronise.
+ *  - ONE STREAM PER HANDLE at a time: the observables share scratch in the handle's workspace (the column
+ *    anchors), so calls on one handle must be ordered (same stream, or the caller's events).  Different
+ *    handles are independent and may run on different streams concurrently.
  *  - The library runs on the current CUDA device and requires compute capability 10.x; there is no
  *    CPU fallback: without a usable device every compute call returns OCT_ECUDA.
  *  - Determinism: the lattice after oct_sweep depends only on (L, seed, init, the sequence of
@@ -91,9 +94,20 @@ int oct_set_state(oct_ctx*, uint64_t t_mcs, int64_t h00, int64_t net, void* stre
  * lasts (1 - N_border/N) MCS of physical time (Eq. (9) :137, R9; see oct_time_per_sweep).
  * oct_sweep(a) followed by oct_sweep(b) equals oct_sweep(a+b).
  * Errors (nothing is enqueued): EINVAL for p,q outside [0,1], unknown dev/blk, cell larger than the
- * domain, blk=DT/DTr with tc<1 (:182), L < 2D, D outside {32,64,128,256} or a (D,TC) pair the library was
- * not built for, t+n_mcs > 2^32-1.  ECUDA: a launch failed (text via oct_last_error). */
+ * domain, blk=DT/DTr with tc<1 (:182), L < 2D for DT/DTr (2D x 2D tiles) or L < D for the dead-border layers,
+ * D outside {32,64,128,256} or a (D,TC) pair the library was not built for, t+n_mcs > 2^32-1.
+ * ECUDA: a launch failed (text via oct_last_error); the sweeps enqueued before the failing one stay enqueued and
+ * oct_mcs() reports how many were. */
 int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* stream);
+
+/* The same n_mcs sweeps on n independent simulations of ONE lattice size at once (ensembles: the paper's curves are
+ * means over n = 20 ... 4367 runs, many at L <= 2^13): every kernel launch covers the
+ * domains of all members (grid = domains x members, at most 64 members per launch), so small lattices fill the
+ * GPU.  Each member keeps its own lattice, counters, seed and clock; its result is bit-identical to what
+ * oct_sweep on that handle alone would give.  Shapes without a many-lattices kernel (D > 64, bit-packed kernel)
+ * run the members one after the other.  The kernel option of handle 0 applies.
+ * Errors: as oct_sweep, plus EINVAL for n = 0, a null or repeated handle, or members of different L. */
+int oct_sweep_batch(oct_ctx* const* handles, uint32_t n, uint64_t n_mcs, double p, double q, int scheme, void* stream);
 
 /* Integrate the slopes into int32 heights h[y*L+x] (:52 "peaks of the octahedra define the height
  * profile"; anchor h(0,0) tracked exactly, R20).  heights_dev holds L*L int32. */
@@ -105,13 +119,13 @@ int oct_heights(oct_ctx*, int32_t* heights_dev, void* stream);
 int oct_width2(oct_ctx*, int64_t* out_dev, void* stream);
 
 /* Waiting-time snapshot for aging (:75-80): copies the packed lattice to lattice_copy_dev
- * (oct_lattice_bytes) and writes anchor_out_dev[2] = {h(0,0), net} at this moment. */
+ * (oct_lattice_bytes, 16-byte aligned) and writes anchor_out_dev[2] = {h(0,0), net} at this moment. */
 int oct_snapshot(oct_ctx*, void* lattice_copy_dev, int64_t* anchor_out_dev, void* stream);
 
 /* Integer sums for the height autocorrelation C_h(t,s) of Eq. (6) :92-98 (R7) between the current
  * lattice and a snapshot: out_dev[5] = {S_t, S_s, S_ts, c_t, c_s}, S_t = sum (h_t-c_t),
  * S_s = sum (h_s-c_s), S_ts = sum (h_t-c_t)(h_s-c_s).  With snapshot == current state the sums
- * reproduce oct_width2's (C_h(s,s) = W^2(s), :97). */
+ * reproduce oct_width2's (C_h(s,s) = W^2(s), :97).  snapshot_dev must be 16-byte aligned (EINVAL otherwise). */
 int oct_autocorr(oct_ctx*, const void* snapshot_dev, const int64_t* snapshot_anchor_dev,
                  int64_t* out_dev, void* stream);
 
@@ -121,6 +135,20 @@ int oct_autocorr(oct_ctx*, const void* snapshot_dev, const int64_t* snapshot_anc
  * the four single sums are L*L/2 for any valid surface).  C_s = oct_cs_from_sums over M = 2 L^2 variables
  * (or M = L^2 for one direction); C_s(s,s) = 1/4. */
 int oct_slope_autocorr(oct_ctx*, const void* snapshot_dev, int64_t* out_dev, void* stream);
+
+/* ONE pass over the current lattice (and the snapshot) for any combination `what` of the observables above:
+ * OCT_OBS_W2 (oct_width2's sums), OCT_OBS_CH (oct_autocorr's), OCT_OBS_CS (oct_slope_autocorr's).  A measurement point
+ * of an aging run wants all three: together they read the lattice and the snapshot once (2 x L^2/4
+ * bytes) instead of five times.  out_dev[16] (int64; all of it is overwritten):
+ *   [0..3] = {S1, S2, c, net}   [4..8] = {S_t, S_s, S_ts, c_t, c_s}   [9..14] = {xx, yy, x_t, y_t, x_s, y_s}   [15] = 0
+ * with the meanings given at oct_width2 / oct_autocorr / oct_slope_autocorr; groups not asked for stay zero.
+ * snapshot_dev (16-byte aligned) is needed for CH and CS, snapshot_anchor_dev for CH; EINVAL otherwise. */
+enum { OCT_OBS_W2 = 1, OCT_OBS_CH = 2, OCT_OBS_CS = 4 };
+int oct_observe(oct_ctx*, int what, const void* snapshot_dev, const int64_t* snapshot_anchor_dev,
+                int64_t* out_dev, void* stream);
+
+/* Copy `bytes` bytes of a device buffer (e.g. the sums above) to host memory.  SYNCHRONISES `stream`. */
+int oct_fetch(oct_ctx*, const void* src_dev, void* dst_host, size_t bytes, void* stream);
 
 /* Copy the packed lattice device -> host (canonical words).  SYNCHRONISES `stream`. */
 int oct_export(oct_ctx*, void* lattice_host, void* stream);

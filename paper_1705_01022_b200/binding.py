@@ -22,7 +22,9 @@ EXPORTS = (
     "oct_width2", "oct_snapshot", "oct_autocorr", "oct_export", "oct_upload", "oct_counters", "oct_mcs",
     "oct_destroy", "oct_strerror", "oct_last_error", "oct_launch_count", "oct_w2_from_sums", "oct_c_from_sums",
     "oct_time_per_sweep", "oct_scheme_supported", "oct_set_option", "oct_slope_autocorr", "oct_cs_from_sums",
+    "oct_sweep_batch", "oct_observe", "oct_fetch",
 )
+OCT_OBS_W2, OCT_OBS_CH, OCT_OBS_CS = 1, 2, 4
 OCT_OPT_KERNEL = 1
 OCT_KERNEL_AUTO, OCT_KERNEL_BITPACKED, OCT_KERNEL_LINKS_B = 0, 1, 2
 
@@ -56,6 +58,7 @@ def load(rebuild_if_stale: bool = True):
         "oct_create": (i32, [C.POINTER(vp), u32, u64, i32, vp, vp, vp]),
         "oct_set_state": (i32, [vp, u64, i64, i64, vp]),
         "oct_sweep": (i32, [vp, u64, dbl, dbl, i32, vp]),
+        "oct_sweep_batch": (i32, [C.POINTER(vp), u32, u64, dbl, dbl, i32, vp]),
         "oct_heights": (i32, [vp, vp, vp]), "oct_width2": (i32, [vp, vp, vp]),
         "oct_snapshot": (i32, [vp, vp, vp, vp]), "oct_autocorr": (i32, [vp, vp, vp, vp, vp]),
         "oct_export": (i32, [vp, vp, vp]), "oct_upload": (i32, [vp, vp, vp]), "oct_counters": (i32, [vp, vp, vp]),
@@ -66,6 +69,7 @@ def load(rebuild_if_stale: bool = True):
         "oct_time_per_sweep": (dbl, [u32, i32]), "oct_scheme_supported": (i32, [u32, i32]),
         "oct_set_option": (i32, [vp, i32, i32]),
         "oct_slope_autocorr": (i32, [vp, vp, vp, vp]), "oct_cs_from_sums": (dbl, [u64, i64, i64, i64]),
+        "oct_observe": (i32, [vp, i32, vp, vp, vp, vp]), "oct_fetch": (i32, [vp, vp, vp, sz, vp]),
     }
     for name in EXPORTS:
         fn = getattr(L, name)          # AttributeError if a declared symbol is not exported
@@ -114,6 +118,15 @@ def _stream_ptr(stream) -> int:
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return int(s.cuda_stream)
+
+
+def oct_sweep_batch(sims, n_mcs: int, p: float, q: float, scheme: int, stream=None):
+    """n_mcs sweeps of every simulation in `sims` (one lattice size), all members in each kernel launch."""
+    sims = list(sims)
+    arr = (C.c_void_p * len(sims))(*[s._h for s in sims])
+    rc = load().oct_sweep_batch(arr, len(sims), n_mcs, p, q, scheme, _stream_ptr(stream))
+    if rc:
+        raise OctError(rc, "oct_sweep_batch", load().oct_last_error(sims[0]._h).decode() if sims else "")
 
 
 class Sim:
@@ -205,6 +218,18 @@ class Sim:
         self._check(self._l.oct_slope_autocorr(self._h, snapshot.data_ptr(), out.data_ptr(), _stream_ptr(stream)),
                     "oct_slope_autocorr")
         return out
+
+    def oct_observe(self, what: int, snapshot=None, anchor=None, out=None, stream=None):
+        """Device tensor int64[16]: [0..3] W^2 sums, [4..8] C_h sums, [9..14] C_s sums (one pass, see oct.h)."""
+        if out is None:
+            out = self.torch.empty(16, dtype=self.torch.int64, device=self.device)
+        self._check(self._l.oct_observe(self._h, what, snapshot.data_ptr() if snapshot is not None else None,
+                                        anchor.data_ptr() if anchor is not None else None, out.data_ptr(), _stream_ptr(stream)),
+                    "oct_observe")
+        return out
+
+    def oct_fetch(self, src, host_ptr: int, nbytes: int, stream=None):
+        self._check(self._l.oct_fetch(self._h, src.data_ptr(), host_ptr, nbytes, _stream_ptr(stream)), "oct_fetch")
 
     def oct_export(self, host=None, stream=None) -> np.ndarray:
         """Canonical packed words as a (L/4, L/4) uint32 numpy array (synchronises)."""

@@ -11,10 +11,16 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboct_b200.so")
-SOURCES = ["oct_api.cu"]
-HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "observe_rows.cuh", "philox.cuh", os.path.join("..", "..", "include", "oct.h")]
+# translation units: (object name, source, extra defines).  sweep_inst.cu is compiled once per kernel family and
+# domain size so that the ~200 kernel instantiations build in parallel.
+UNITS = [("oct_api", "oct_api.cu", [])] + \
+        [(f"packed_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=0", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7, 8)] + \
+        [(f"links_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=1", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7)]
+HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "observe_rows.cuh", "philox.cuh", "launch.h", "sweep_inst.cu", "oct_api.cu",
+           os.path.join("..", "..", "include", "oct.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "--use_fast_math", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC,-O2,-Wall", "--use_fast_math", "-Xptxas", "-v"]
+OBJDIR = os.path.join(HERE, "build")
 
 
 def nvcc() -> str:
@@ -28,25 +34,47 @@ def stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    deps = [os.path.join(CSRC, f) for f in HEADERS] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, ptxas_info: str | None = None) -> str:
-    """ptxas_info: optional path that receives ptxas' per-kernel register / spill / shared-memory report."""
-    if force or stale():
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc(), *NVCC_FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or res.returncode:
-            print(res.stdout)
-            print(res.stderr)
+def build(force: bool = False, verbose: bool = False, ptxas_info: str | None = None, extra_flags=()) -> str:
+    """Compile every unit (in parallel), link liboct_b200.so.  ptxas_info: optional path that receives ptxas'
+    per-kernel register / spill / shared-memory report; extra_flags: additional nvcc flags (e.g. -D switches)."""
+    if not (force or stale()):
+        return LIB
+    os.makedirs(OBJDIR, exist_ok=True)
+    tag = f".tmp{os.getpid()}"
+    procs = []
+    for name, src, defs in UNITS:
+        obj = os.path.join(OBJDIR, name + tag + ".o")
+        cmd = [nvcc(), *NVCC_FLAGS, *defs, *extra_flags, "-c", "-o", obj, os.path.join(CSRC, src)]
+        procs.append((name, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
+    report, failed, objs = [], None, []
+    for name, obj, pr in procs:
+        out, err = pr.communicate()
+        report.append(err)
+        objs.append(obj)
+        if verbose or pr.returncode:
+            print(out)
+            print(err)
+        if pr.returncode and failed is None:
+            failed = f"nvcc failed on {name}:\n" + err[-4000:]
+    try:
+        if failed:
+            raise RuntimeError(failed)
+        tmp = LIB + tag
+        res = subprocess.run([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs], capture_output=True, text=True)
         if res.returncode:
-            raise RuntimeError("nvcc failed:\n" + res.stderr[-4000:])
+            raise RuntimeError("link failed:\n" + res.stderr[-4000:])
         if ptxas_info:
             with open(ptxas_info, "w") as f:
-                f.write("".join(l for l in res.stderr.splitlines(True) if "Compile time" not in l))
+                f.write("".join(l for e in report for l in e.splitlines(True) if "Compile time" not in l))
         os.replace(tmp, LIB)
+    finally:
+        for o in objs:
+            if os.path.exists(o):
+                os.unlink(o)
     return LIB
 
 

@@ -66,7 +66,6 @@ column_anchor_kernel(const uint32_t* __restrict__ lat, uint32_t L, int32_t* __re
 }
 
 // ---- kernel 2 -------------------------------------------------------------------------------------
-enum : int { kModeHeights = 0, kModeWidth2 = 1, kModeAutocorr = 2 };
 
 struct RowsParams {
     const uint32_t* latA;        // current lattice
@@ -75,8 +74,8 @@ struct RowsParams {
     const int32_t* anchorB;
     const unsigned long long* countersA;    // [0] net, [1] h00 of the current lattice
     const long long* snapB;                 // {h00, net} of the snapshot
-    int32_t* heights;                       // kModeHeights output
-    unsigned long long* out;                // kModeWidth2: {S1,S2,c,net}; kModeAutocorr: {St,Ss,Sts,ct,cs}
+    int32_t* heights;                       // heights_kernel output
+    unsigned long long* out;                // rows3_kernel: [0..3] W^2 sums, [4..8] C_h sums, [9..14] C_s sums
     uint32_t L;
 };
 

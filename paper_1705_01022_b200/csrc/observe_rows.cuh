@@ -87,24 +87,53 @@ __device__ __forceinline__ void load_run(const uint32_t* __restrict__ p, uint32_
 
 constexpr int kRows2Warps = 8;
 
-// RUN words per lane per chunk: 16 for L >= 2048 (chunk = 512 words), 4 below (any L >= 16 works:
-// lanes beyond L/16 idle).
-template <int MODE, int RUN>
-__global__ void __launch_bounds__(kRows2Warps * 32) rows2_kernel(const RowsParams P)
+// what one pass computes (oct_observe): any combination
+enum : int { kObsW2 = 1, kObsCh = 2, kObsCs = 4 };
+
+// the four sigma_x bits of every site row of a word, one per byte lane: b[i] byte j = sigma_x(site i of row j)
+__device__ __forceinline__ void slope_bytes(uint32_t w, uint32_t (&b)[4])
 {
-    static_assert(MODE == kModeWidth2 || MODE == kModeAutocorr, "heights are written by heights_kernel");
+    b[0] = w & kOnes; b[1] = (w >> 2) & kOnes; b[2] = (w >> 4) & kOnes; b[3] = (w >> 6) & kOnes;
+}
+
+// heights of the four sites of a word, byte-parallel over its four site rows, from the heights just west of it:
+// H_i = H_{i-1} + 2 b_i - 1 (bytes stay within [1, 255]: no borrow between byte lanes).  The subtraction issues on
+// the ALU pipe, the multiply-add on the FMA pipe; the last H is the west height of the next word.
+__device__ __forceinline__ void walk_word(uint32_t w, uint32_t& west, uint32_t (&H)[4])
+{
+    uint32_t b[4];
+    slope_bytes(w, b);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        H[i] = b[i] * 2u + (west - kOnes);
+        west = H[i];
+    }
+}
+
+// One pass over the packed lattice (and the snapshot) for any combination of
+//   kObsW2: S1 = sum (h - c), S2 = sum (h - c)^2                         (Eq. (3) :61)
+//   kObsCh: S_t = S1, S_s = sum (h_s - c_s), S_ts = sum (h - c)(h_s - c_s) (Eq. (6) :92-98)
+//   kObsCs: the six slope-bit sums of :85-88
+// RUN words per lane per chunk: 16 for L >= 2048 (chunk = 512 words), 4 below (any L >= 16 works: lanes beyond L/16 idle).
+// out (int64): [0..3] = {S1, S2, c, net}; [4..8] = {S_t, S_s, S_ts, c_t, c_s}; [9..14] = {xx, yy, x_t, y_t, x_s, y_s}
+template <int WHAT, int RUN>
+__global__ void __launch_bounds__(kRows2Warps * 32) rows3_kernel(const RowsParams P)
+{
+    constexpr bool W2 = (WHAT & kObsW2) != 0, CH = (WHAT & kObsCh) != 0, CS = (WHAT & kObsCs) != 0;
+    constexpr bool NEED_B = CH || CS;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t LW = P.L >> 2;
     const uint32_t wy = blockIdx.x * kRows2Warps + warp;     // word-row of this warp
-    long long s1 = 0, s2 = 0, s3 = 0;
+    long long s1 = 0, s2 = 0, ss = 0, sts = 0;
+    unsigned int pc[6] = {0, 0, 0, 0, 0, 0};                 // per thread < 2^32 bits: a thread sees L/8 words of 32 bits per row chunk
 
     if (wy < LW) {
         const uint32_t* rowA = P.latA + (size_t)wy * LW;
-        const uint32_t* rowB = MODE == kModeAutocorr ? P.latB + (size_t)wy * LW : nullptr;
+        const uint32_t* rowB = NEED_B ? P.latB + (size_t)wy * LW : nullptr;
         // height just west of site 0 of site row 4*wy, relative to h(0,0):  h(-1,y) = h(0,y) - sigma_x(0,y)
-        int carryA = P.anchorA[4 * wy] - ((rowA[0] & 1u) ? 1 : -1);
-        int carryB = 0;
-        if constexpr (MODE == kModeAutocorr) carryB = P.anchorB[4 * wy] - ((rowB[0] & 1u) ? 1 : -1);
+        int carryA = 0, carryB = 0;
+        if constexpr (W2 || CH) carryA = P.anchorA[4 * wy] - ((rowA[0] & 1u) ? 1 : -1);
+        if constexpr (CH) carryB = P.anchorB[4 * wy] - ((rowB[0] & 1u) ? 1 : -1);
         const uint32_t lanes_used = LW / RUN < 32u ? LW / RUN : 32u;
         const bool on = (uint32_t)lane < lanes_used;
 
@@ -113,96 +142,113 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows2_kernel(const RowsParam
             uint32_t wa[RUN], wb[RUN];
             if (on) {
                 load_run<RUN>(rowA + wx, wa);
-                if constexpr (MODE == kModeAutocorr) load_run<RUN>(rowB + wx, wb);
+                if constexpr (NEED_B) load_run<RUN>(rowB + wx, wb);
             } else {
 #pragma unroll
                 for (int k = 0; k < RUN; ++k) { wa[k] = 0x05050505u; wb[k] = 0x05050505u; }   // zero net slope
             }
-
-            {
-                // heights relative to the (still unknown) height s at the start of this lane's run, kept ENTIRELY
-                // in bytes: over a run of <= 64 sites they stay within +-73 of s, so H = e - s + 128 is an
-                // unsigned byte and the run's sums are plain DP4A accumulations; the bias comes off once per run
+            if constexpr (CS) {
+                if (on) {
+                    constexpr uint32_t MX = 0x55555555u;
+#pragma unroll
+                    for (int k = 0; k < RUN; ++k) {
+                        const uint32_t ab = wa[k] & wb[k];
+                        pc[0] += __popc(ab & MX); pc[1] += __popc(ab);           // [1], [3], [5] hold x + y until the end
+                        pc[2] += __popc(wa[k] & MX); pc[3] += __popc(wa[k]);
+                        pc[4] += __popc(wb[k] & MX); pc[5] += __popc(wb[k]);
+                    }
+                }
+            }
+            if constexpr (W2 || CH) {
+                // heights relative to the (still unknown) height s at the start of this lane's run, kept ENTIRELY in bytes:
+                // over a run of <= 64 sites they stay within +-73 of s, so H = e - s + 128 is an unsigned byte and the
+                // run's sums are plain DP4A accumulations; the bias comes off once per run
                 uint32_t ba = run_start_dq(wa[0]) + 112u * kOnes, bb = 0;      // bytes left_j - s + 128
-                if constexpr (MODE == kModeAutocorr) bb = run_start_dq(wb[0]) + 112u * kOnes;
-                unsigned int a1 = 0, b1 = 0, qq = 0;     // sum H_A, sum H_B, sum H_A^2 (Width2) or sum H_A H_B (Autocorr)
+                if constexpr (CH) bb = run_start_dq(wb[0]) + 112u * kOnes;
+                unsigned int a1 = 0, b1 = 0, qa = 0, qab = 0;                  // sum H_A, sum H_B, sum H_A^2, sum H_A H_B
 #pragma unroll
                 for (int k = 0; k < RUN; ++k) {
-                    uint32_t PA[4], HA[4];
-                    prefix_counts(wa[k], PA);
+                    uint32_t HA[4], HB[4];
+                    walk_word(wa[k], ba, HA);
+                    if constexpr (CH) walk_word(wb[k], bb, HB);
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) { HA[i] = ba - (uint32_t)(i + 1) * kOnes + 2u * PA[i]; a1 = __dp4a(HA[i], kOnes, a1); }
-                    ba = ba + 2u * PA[3] - 4u * kOnes;
-                    if constexpr (MODE == kModeWidth2) {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) qq = __dp4a(HA[i], HA[i], qq);
-                    } else {
-                        uint32_t PB[4], HB[4];
-                        prefix_counts(wb[k], PB);
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            HB[i] = bb - (uint32_t)(i + 1) * kOnes + 2u * PB[i];
-                            b1 = __dp4a(HB[i], kOnes, b1);
-                            qq = __dp4a(HA[i], HB[i], qq);
-                        }
-                        bb = bb + 2u * PB[3] - 4u * kOnes;
+                    for (int i = 0; i < 4; ++i) {
+                        a1 = __dp4a(HA[i], kOnes, a1);
+                        if constexpr (W2) qa = __dp4a(HA[i], HA[i], qa);
+                        if constexpr (CH) { b1 = __dp4a(HB[i], kOnes, b1); qab = __dp4a(HA[i], HB[i], qab); }
                     }
                 }
                 constexpr int nn = 16 * RUN;
+                constexpr long long n = 16 * RUN;
                 const int ra1 = (int)a1 - 128 * nn;                                   // sum (e_A - s_A)
                 const int rb1 = (int)b1 - 128 * nn;
-                // Width2: sum (H-128)^2 ; Autocorr: sum (H_A-128)(H_B-128)
-                const int q = MODE == kModeWidth2 ? (int)(qq - 256u * a1) + 16384 * nn : (int)(qq - 128u * (a1 + b1)) + 16384 * nn;
                 const int totA = (int)(ba & 0xFFu) - 128, totB = (int)(bb & 0xFFu) - 128;   // net slope of site row 0 over the run
                 // place the runs: exclusive scan of the runs' net slope of site row 0
                 const int inclA = warp_inclusive_scan_i32(totA, lane);
                 const long long sA = carryA + inclA - totA;
                 carryA += __shfl_sync(0xFFFFFFFFu, inclA, 31);
-                constexpr long long n = 16 * RUN;
-                if constexpr (MODE == kModeWidth2) {
-                    if (on) {
-                        s1 += n * sA + ra1;
-                        s2 += n * sA * sA + 2 * sA * ra1 + q;
-                    }
-                } else {
+                if (on) s1 += n * sA + ra1;
+                if constexpr (W2) {
+                    const int q = (int)(qa - 256u * a1) + 16384 * nn;                 // sum (H - 128)^2
+                    if (on) s2 += n * sA * sA + 2 * sA * ra1 + q;
+                }
+                if constexpr (CH) {
+                    const int q = (int)(qab - 128u * (a1 + b1)) + 16384 * nn;         // sum (H_A - 128)(H_B - 128)
                     const int inclB = warp_inclusive_scan_i32(totB, lane);
                     const long long sB = carryB + inclB - totB;
                     carryB += __shfl_sync(0xFFFFFFFFu, inclB, 31);
                     if (on) {
-                        s1 += n * sA + ra1;
-                        s2 += n * sB + rb1;
-                        s3 += n * sA * sB + sA * rb1 + sB * ra1 + q;
+                        ss += n * sB + rb1;
+                        sts += n * sA * sB + sA * rb1 + sB * ra1 + q;
                     }
                 }
             }
         }
     }
 
-    if constexpr (MODE != kModeHeights) {
-        __shared__ long long red[3][kRows2Warps];
+    __shared__ long long red[4][kRows2Warps];
+    __shared__ unsigned long long redc[6][kRows2Warps];
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            s1 += __shfl_xor_sync(0xFFFFFFFFu, s1, off);
-            s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, off);
-            if constexpr (MODE == kModeAutocorr) s3 += __shfl_xor_sync(0xFFFFFFFFu, s3, off);
+    for (int off = 16; off > 0; off >>= 1) {
+        s1 += __shfl_xor_sync(0xFFFFFFFFu, s1, off);
+        if constexpr (W2) s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, off);
+        if constexpr (CH) { ss += __shfl_xor_sync(0xFFFFFFFFu, ss, off); sts += __shfl_xor_sync(0xFFFFFFFFu, sts, off); }
+    }
+    if constexpr (CS) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const unsigned long long v = __reduce_add_sync(0xFFFFFFFFu, pc[k]);   // a warp's total per row stays far below 2^32
+            if (lane == 0) redc[k][warp] = v;
         }
-        if (lane == 0) { red[0][warp] = s1; red[1][warp] = s2; red[2][warp] = s3; }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            long long t1 = 0, t2 = 0, t3 = 0;
-            for (int w = 0; w < kRows2Warps; ++w) { t1 += red[0][w]; t2 += red[1][w]; t3 += red[2][w]; }
+    }
+    if (lane == 0) { red[0][warp] = s1; red[1][warp] = s2; red[2][warp] = ss; red[3][warp] = sts; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long t1 = 0, t2 = 0, t3 = 0, t4 = 0;
+        for (int w = 0; w < kRows2Warps; ++w) { t1 += red[0][w]; t2 += red[1][w]; t3 += red[2][w]; t4 += red[3][w]; }
+        if constexpr (W2) {
             atomicAdd(&P.out[0], (unsigned long long)t1);
             atomicAdd(&P.out[1], (unsigned long long)t2);
-            if constexpr (MODE == kModeAutocorr) atomicAdd(&P.out[2], (unsigned long long)t3);
-            if (blockIdx.x == 0) {
-                if constexpr (MODE == kModeWidth2) {
-                    P.out[2] = P.countersA[1];             // c = h(0,0)
-                    P.out[3] = P.countersA[0];             // net
-                } else {
-                    P.out[3] = P.countersA[1];             // c_t
-                    P.out[4] = (unsigned long long)P.snapB[0];   // c_s
-                }
-            }
+        }
+        if constexpr (CH) {
+            atomicAdd(&P.out[4], (unsigned long long)t1);
+            atomicAdd(&P.out[5], (unsigned long long)t3);
+            atomicAdd(&P.out[6], (unsigned long long)t4);
+        }
+        if (blockIdx.x == 0) {
+            if constexpr (W2) { P.out[2] = P.countersA[1]; P.out[3] = P.countersA[0]; }                         // c = h(0,0), net
+            if constexpr (CH) { P.out[7] = P.countersA[1]; P.out[8] = (unsigned long long)P.snapB[0]; }         // c_t, c_s
+        }
+    }
+    if constexpr (CS) {
+        if (threadIdx.x < 6) {
+            unsigned long long t = 0;
+            for (int w = 0; w < kRows2Warps; ++w) t += redc[threadIdx.x][w];
+            // [1], [3], [5] were counted over both slope bits: take the x part off
+            unsigned long long tx = 0;
+            if (threadIdx.x & 1) { for (int w = 0; w < kRows2Warps; ++w) tx += redc[threadIdx.x - 1][w]; }
+            const int slot = 9 + (int)threadIdx.x;
+            atomicAdd(&P.out[slot], t - tx);
         }
     }
 }

@@ -13,8 +13,8 @@
 #include "observe.cuh"
 #include "observe_rows.cuh"
 #include "philox.cuh"
+#include "launch.h"
 #include "sweep.cuh"
-#include "sweep_links.cuh"
 
 using namespace octb;
 
@@ -61,84 +61,26 @@ int fail_cuda(oct_ctx* c, cudaError_t e, const char* what)
         if (e__ != cudaSuccess) return fail_cuda(ctx, e__, #call);  \
     } while (0)
 
-// ---- sweep kernel dispatch ---------------------------------------------------------------------------
-struct SweepLaunch {
-    void (*kern)(const SweepParams);
-    int threads, smem, dpb;
-};
-
-#ifndef OCT_CELLS_PER_WARP
-#define OCT_CELLS_PER_WARP 128   // bit-packed kernel: cells carried by one warp (4 per lane; 8 overflows the instruction cache, profiles/r1_a)
-#endif
-constexpr int pick_wpd(int log2d, int tcx, int tcy)
-{
-    const int ncell = ((1 << log2d) / (4 << tcx)) * ((1 << log2d) / (4 << tcy));
-    return ncell <= OCT_CELLS_PER_WARP ? 1 : ncell / OCT_CELLS_PER_WARP;
-}
-
-template <int LD, int TX, int TY, int BLK>
-SweepLaunch make_launch()
-{
-    constexpr int W = pick_wpd(LD, TX, TY);
-    using SH = SweepShape<LD, TX, TY, W>;
-    return SweepLaunch{sweep_kernel<LD, TX, TY, BLK, W>, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
-}
-
-// (log2 D, tcx, tcy) combinations the library is built for
-#define OCT_SHAPES(X)                                                      \
-    X(5, 0, 0) X(5, 1, 1) X(5, 2, 2)                                       \
-    X(6, 0, 0) X(6, 1, 1) X(6, 2, 2) X(6, 2, 1) X(6, 3, 1) X(6, 1, 3)      \
-    X(7, 0, 0) X(7, 1, 1) X(7, 2, 2) X(7, 2, 1) X(7, 3, 2) X(7, 4, 1)      \
-    X(8, 1, 1) X(8, 2, 2) X(8, 2, 1) X(8, 3, 2) X(8, 4, 1)
-
+// ---- sweep kernel dispatch (the kernels are instantiated in sweep_inst.cu, one object per family and size) ----
 bool find_launch(int ld, int tx, int ty, int blk, SweepLaunch* out)
 {
-#define X(LD, TX, TY)                                                               \
-    if (ld == LD && tx == TX && ty == TY) {                                         \
-        if (blk == kBlkSync) { *out = make_launch<LD, TX, TY, kBlkSync>(); return true; }       \
-        if (blk == kBlkDelayed) { *out = make_launch<LD, TX, TY, kBlkDelayed>(); return true; } \
-        if constexpr (TX >= 1 && TY >= 1) {                                         \
-            if (blk == kBlkDT) { *out = make_launch<LD, TX, TY, kBlkDT>(); return true; }       \
-        }                                                                           \
-        return false;                                                               \
+    switch (ld) {
+        case 5: return oct_find_packed_5(tx, ty, blk, out);
+        case 6: return oct_find_packed_6(tx, ty, blk, out);
+        case 7: return oct_find_packed_7(tx, ty, blk, out);
+        case 8: return oct_find_packed_8(tx, ty, blk, out);
+        default: return false;
     }
-    OCT_SHAPES(X)
-#undef X
-    return false;
 }
-
-// ---- link-entry sweep kernel (sweep_links.cuh): DTr/DT device layer, D <= 128 ------------------------
-template <int LD, int TX, int TY, int BLK, int W, int DPB>
-SweepLaunch make_links_launch(bool dead)
-{
-    using SH = LinkShape<LD, TX, TY, W, DPB>;
-    return SweepLaunch{dead ? sweep_links_kernel<LD, TX, TY, BLK, W, DPB, true> : sweep_links_kernel<LD, TX, TY, BLK, W, DPB, false>,
-                       SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
-}
-
-// (log2 D, tcx, tcy, warps per domain, domains per CTA): variant A is the default (the faster one on
-// B200: D=64 one warp per domain, two cells per lane, warp-level sync only; D=128 eight warps), variant
-// B the alternative work split of the two headline shapes
-#define OCT_LINK_SHAPES_A(X)                                                         \
-    X(5, 0, 0, 1, 4) X(6, 0, 0, 4, 1) X(6, 1, 1, 1, 4) X(6, 2, 1, 1, 4)              \
-    X(7, 0, 0, 8, 1) X(7, 1, 1, 8, 1) X(7, 2, 2, 2, 1) X(7, 2, 1, 4, 1) X(7, 3, 2, 1, 1) X(7, 4, 1, 1, 1)
-#define OCT_LINK_SHAPES_B(X) X(6, 1, 1, 2, 2) X(7, 1, 1, 4, 1)
 
 bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out)
 {
-#define X(LD, TX, TY, W, DPB)                                                                        \
-    if (ld == LD && tx == TX && ty == TY) {                                                          \
-        if (blk == kBlkSync) { *out = make_links_launch<LD, TX, TY, kBlkSync, W, DPB>(dead); return true; }       \
-        if (blk == kBlkDelayed) { *out = make_links_launch<LD, TX, TY, kBlkDelayed, W, DPB>(dead); return true; } \
-        if constexpr (TX >= 1 && TY >= 1) {                                                          \
-            if (blk == kBlkDT) { *out = make_links_launch<LD, TX, TY, kBlkDT, W, DPB>(dead); return true; }       \
-        }                                                                                            \
-        return false;                                                                                \
+    switch (ld) {
+        case 5: return oct_find_links_5(tx, ty, blk, variant_b, dead, out);
+        case 6: return oct_find_links_6(tx, ty, blk, variant_b, dead, out);
+        case 7: return oct_find_links_7(tx, ty, blk, variant_b, dead, out);
+        default: return false;
     }
-    if (variant_b) { OCT_LINK_SHAPES_B(X) }
-    OCT_LINK_SHAPES_A(X)
-#undef X
-    return false;
 }
 
 struct SchemeFields { uint32_t dev, blk, tcx, tcy, log2D; };
@@ -160,7 +102,9 @@ int check_scheme(uint32_t L, int scheme)
     if (cx > D || cy > D || cx > 64 || cy > 64) return OCT_EINVAL;
     const bool blk_dt = f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR;
     if (blk_dt && (f.tcx < 1 || f.tcy < 1)) return OCT_EINVAL;   // :182
-    if (L < 2 * D) return OCT_EINVAL;   // window (D/4+1 words) must not wrap onto itself
+    // DT / DTr tile the lattice with 2D x 2D tiles; the dead-border layers with D x D tiles (a single tile, L = D, is
+    // allowed: its window wraps onto itself only in the dead rim, which is neither tested nor written back)
+    if (f.dev <= OCT_DEV_DT ? L < 2 * D : L < D) return OCT_EINVAL;
     SweepLaunch sl;
     if (!find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk_dt ? kBlkDT : kBlkSync, &sl)) return OCT_EINVAL;
     return OCT_OK;
@@ -182,12 +126,26 @@ int ensure_device(oct_ctx* c)
 }
 
 // one warp per word-row; 16 words per lane per chunk once a row holds at least one full chunk
-template <int MODE>
-void launch_rows(const RowsParams& rp, uint32_t LW, cudaStream_t st)
+template <int WHAT>
+void launch_rows_what(const RowsParams& rp, uint32_t LW, cudaStream_t st)
 {
     const unsigned blocks = (LW + kRows2Warps - 1) / kRows2Warps;
-    if (LW >= 512u) rows2_kernel<MODE, 16><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
-    else            rows2_kernel<MODE, 4><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
+    if (LW >= 512u) rows3_kernel<WHAT, 16><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
+    else            rows3_kernel<WHAT, 4><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
+}
+
+void launch_rows(int what, const RowsParams& rp, uint32_t LW, cudaStream_t st)
+{
+    switch (what) {
+        case 1: launch_rows_what<1>(rp, LW, st); break;
+        case 2: launch_rows_what<2>(rp, LW, st); break;
+        case 3: launch_rows_what<3>(rp, LW, st); break;
+        case 4: launch_rows_what<4>(rp, LW, st); break;
+        case 5: launch_rows_what<5>(rp, LW, st); break;
+        case 6: launch_rows_what<6>(rp, LW, st); break;
+        case 7: launch_rows_what<7>(rp, LW, st); break;
+        default: break;
+    }
 }
 
 int launch_anchor(oct_ctx* c, const uint32_t* lat, int32_t* anchor, cudaStream_t st)
@@ -255,46 +213,132 @@ int oct_set_option(oct_ctx* c, int option, int value)
     return OCT_EINVAL;
 }
 
+}  // extern "C"
+
+namespace {
+
+// Everything about a sweep call that does not depend on the lattice it runs on.
+struct SweepPlan {
+    SchemeFields f;
+    SweepLaunch sl;
+    uint32_t P16, Q16, ndom, grid, n_launch;
+};
+
+int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
+{
+    if (!(p >= 0.0 && p <= 1.0) || !(q >= 0.0 && q <= 1.0)) return OCT_EINVAL;
+    if (check_scheme(c->L, scheme) != OCT_OK) return OCT_EINVAL;
+    pl->f = split_scheme(scheme);
+    const SchemeFields& f = pl->f;
+    pl->P16 = prob16(p); pl->Q16 = prob16(q);
+    const int blk = (f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR) ? kBlkDT
+                  : (f.blk == OCT_BLK_DB_DELAYED || (pl->P16 > 0 && pl->Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
+    // the link-entry kernel serves domains that fit shared memory unpacked; the bit-packed kernel serves
+    // everything else (D = 256, domains with fewer than 16 cells)
+    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED &&
+                       find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B,
+                                         f.dev > OCT_DEV_DT, &pl->sl);
+    if (!links && !find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &pl->sl)) return OCT_EINVAL;
+    const bool tiled = f.dev <= OCT_DEV_DT;
+    const uint32_t nt = tiled ? c->L >> (f.log2D + 1) : c->L >> f.log2D;
+    pl->ndom = nt * nt;
+    pl->grid = (pl->ndom + pl->sl.dpb - 1) / pl->sl.dpb;
+    pl->n_launch = tiled ? 4u : (f.dev == OCT_DEV_DBH ? 2u : 1u);   // :144 one launch per domain set; DBh: two intervals (R27)
+    return OCT_OK;
+}
+
+// kernels that need more than 48 KiB of dynamic shared memory are opted in once per function
+int opt_in_smem(oct_ctx* c, const void* fn, int smem)
+{
+    static const void* done[64];
+    static int n_done = 0;
+    if (smem <= 48 * 1024) return OCT_OK;
+    for (int i = 0; i < n_done; ++i) if (done[i] == fn) return OCT_OK;
+    OCT_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    if (n_done < 64) done[n_done++] = fn;
+    return OCT_OK;
+}
+
+void fill_common(SweepParams& sp, const oct_ctx* c, const SweepPlan& pl)
+{
+    sp.L = c->L; sp.log2L = c->log2L; sp.P16 = pl.P16; sp.Q16 = pl.Q16; sp.dev = pl.f.dev; sp.ndom = pl.ndom;
+    sp.dtr_mask = pl.f.blk == OCT_BLK_DTR ? ~0u : 0u;
+}
+
+}  // namespace
+
+extern "C" {
+
 int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* stream)
 {
     if (!c) return OCT_EINVAL;
-    if (!(p >= 0.0 && p <= 1.0) || !(q >= 0.0 && q <= 1.0)) return OCT_EINVAL;
-    if (check_scheme(c->L, scheme) != OCT_OK) return OCT_EINVAL;
+    SweepPlan pl;
+    int rc = plan_sweep(c, p, q, scheme, &pl);
+    if (rc) return rc;
     if (c->t + n_mcs > 0xFFFFFFFFull || c->t + n_mcs < c->t) return OCT_EINVAL;
-    const SchemeFields f = split_scheme(scheme);
-    const uint32_t P16 = prob16(p), Q16 = prob16(q);
-    const int blk = (f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR) ? kBlkDT
-                  : (f.blk == OCT_BLK_DB_DELAYED || (P16 > 0 && Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
-    SweepLaunch sl;
-    // the link-entry kernel serves domains that fit shared memory unpacked; the bit-packed kernel serves
-    // everything else (D = 256, domains with fewer than 32 cells)
-    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED &&
-                       find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B,
-                                         f.dev > OCT_DEV_DT, &sl);
-    if (!links && !find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &sl)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (sl.smem > 48 * 1024)
-        OCT_CUDA(c, cudaFuncSetAttribute(sl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, sl.smem));
-
-    const bool tiled = f.dev <= OCT_DEV_DT;
-    const uint32_t nt = tiled ? c->L >> (f.log2D + 1) : c->L >> f.log2D;
-    const uint32_t ndom = nt * nt;
-    const uint32_t grid = (ndom + sl.dpb - 1) / sl.dpb;
+    rc = opt_in_smem(c, reinterpret_cast<const void*>(pl.sl.kern), pl.sl.smem);
+    if (rc) return rc;
 
     SweepParams sp{};
-    sp.lat = c->lat; sp.counters = c->counters(); sp.L = c->L; sp.log2L = c->log2L;
-    sp.P16 = P16; sp.Q16 = Q16; sp.dev = f.dev; sp.ndom = ndom; sp.rk = c->rk;
-    sp.dtr_mask = f.blk == OCT_BLK_DTR ? ~0u : 0u;
+    fill_common(sp, c, pl);
+    sp.lat = c->lat; sp.counters = c->counters(); sp.rk = c->rk;
     for (uint64_t i = 0; i < n_mcs; ++i) {
         sp.t = static_cast<uint32_t>(c->t);
-        const uint32_t n_launch = tiled ? 4u : (f.dev == OCT_DEV_DBH ? 2u : 1u);   // DBh: two intervals (R27)
-        for (uint32_t si = 0; si < n_launch; ++si) {   // :144 sync = kernel boundary after each set
+        for (uint32_t si = 0; si < pl.n_launch; ++si) {   // :144 sync = kernel boundary after each set
             sp.si = si;
-            sl.kern<<<grid, sl.threads, sl.smem, st>>>(sp);
+            pl.sl.kern<<<pl.grid, pl.sl.threads, pl.sl.smem, st>>>(sp);
             c->launches++;
         }
-        OCT_CUDA(c, cudaGetLastError());
+        OCT_CUDA(c, cudaGetLastError());   // on failure the clock stays at the sweeps completed so far (oct_mcs)
         c->t++;
+    }
+    return OCT_OK;
+}
+
+int oct_sweep_batch(oct_ctx* const* cs, uint32_t n, uint64_t n_mcs, double p, double q, int scheme, void* stream)
+{
+    if (!cs || n == 0) return OCT_EINVAL;
+    for (uint32_t i = 0; i < n; ++i) {
+        if (!cs[i] || cs[i]->L != cs[0]->L) return OCT_EINVAL;
+        if (cs[i]->t + n_mcs > 0xFFFFFFFFull || cs[i]->t + n_mcs < cs[i]->t) return OCT_EINVAL;
+        for (uint32_t j = 0; j < i; ++j) if (cs[j] == cs[i] || cs[j]->lat == cs[i]->lat) return OCT_EINVAL;
+    }
+    oct_ctx* c0 = cs[0];
+    SweepPlan pl;
+    int rc = plan_sweep(c0, p, q, scheme, &pl);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!pl.sl.kern_batch) {
+        // no many-lattices kernel for this shape: the members run one after the other (same results)
+        for (uint32_t i = 0; i < n; ++i) {
+            const int keep = cs[i]->opt_kernel;
+            cs[i]->opt_kernel = c0->opt_kernel;
+            rc = oct_sweep(cs[i], n_mcs, p, q, scheme, stream);
+            cs[i]->opt_kernel = keep;
+            if (rc) return rc;
+        }
+        return OCT_OK;
+    }
+    rc = opt_in_smem(c0, reinterpret_cast<const void*>(pl.sl.kern_batch), pl.sl.smem);
+    if (rc) return rc;
+    SweepBatchParams bp{};
+    fill_common(bp.common, c0, pl);
+    for (uint64_t i = 0; i < n_mcs; ++i) {
+        for (uint32_t m0 = 0; m0 < n; m0 += kMaxBatch) {         // at most kMaxBatch members per launch
+            const uint32_t nb = n - m0 < (uint32_t)kMaxBatch ? n - m0 : (uint32_t)kMaxBatch;
+            for (uint32_t m = 0; m < nb; ++m) {
+                const oct_ctx* c = cs[m0 + m];
+                bp.m[m] = BatchMember{c->lat, c->counters(), (uint32_t)c->seed, (uint32_t)(c->seed >> 32), (uint32_t)c->t, 0u};
+            }
+            for (uint32_t si = 0; si < pl.n_launch; ++si) {
+                bp.common.si = si;
+                pl.sl.kern_batch<<<dim3(pl.grid, nb), pl.sl.threads, pl.sl.smem, st>>>(bp);
+                c0->launches++;
+            }
+        }
+        OCT_CUDA(c0, cudaGetLastError());
+        for (uint32_t m = 0; m < n; ++m) cs[m]->t++;
     }
     return OCT_OK;
 }
@@ -325,7 +369,7 @@ int oct_width2(oct_ctx* c, int64_t* out_dev, void* stream)
     rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters();
     rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
     const uint32_t LW = c->L >> 2;
-    launch_rows<kModeWidth2>(rp, LW, st);
+    launch_rows(kObsW2, rp, LW, st);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;
@@ -333,7 +377,7 @@ int oct_width2(oct_ctx* c, int64_t* out_dev, void* stream)
 
 int oct_snapshot(oct_ctx* c, void* lattice_copy_dev, int64_t* anchor_out_dev, void* stream)
 {
-    if (!c || !lattice_copy_dev || !anchor_out_dev) return OCT_EINVAL;
+    if (!c || !lattice_copy_dev || !anchor_out_dev || (reinterpret_cast<uintptr_t>(lattice_copy_dev) & 15u)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     OCT_CUDA(c, cudaMemcpyAsync(lattice_copy_dev, c->lat, oct_lattice_bytes(c->L), cudaMemcpyDeviceToDevice, st));
     snapshot_anchor_kernel<<<1, 1, 0, st>>>(c->counters(), reinterpret_cast<long long*>(anchor_out_dev));
@@ -344,7 +388,7 @@ int oct_snapshot(oct_ctx* c, void* lattice_copy_dev, int64_t* anchor_out_dev, vo
 
 int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_anchor_dev, int64_t* out_dev, void* stream)
 {
-    if (!c || !snapshot_dev || !snapshot_anchor_dev || !out_dev) return OCT_EINVAL;
+    if (!c || !snapshot_dev || !snapshot_anchor_dev || !out_dev || (reinterpret_cast<uintptr_t>(snapshot_dev) & 15u)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 5 * sizeof(int64_t), st));
     int rc = launch_anchor(c, c->lat, c->anchorA(), st);
@@ -355,9 +399,9 @@ int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_a
     rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
     rp.anchorA = c->anchorA(); rp.anchorB = c->anchorB(); rp.countersA = c->counters();
     rp.snapB = reinterpret_cast<const long long*>(snapshot_anchor_dev);
-    rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
+    rp.out = reinterpret_cast<unsigned long long*>(out_dev) - 4; rp.L = c->L;      // the kernel writes slots 4..8
     const uint32_t LW = c->L >> 2;
-    launch_rows<kModeAutocorr>(rp, LW, st);
+    launch_rows(kObsCh, rp, LW, st);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;
@@ -375,6 +419,39 @@ int oct_slope_autocorr(oct_ctx* c, const void* snapshot_dev, int64_t* out_dev, v
                                                            n_vec, reinterpret_cast<unsigned long long*>(out_dev));
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_observe(oct_ctx* c, int what, const void* snapshot_dev, const int64_t* snapshot_anchor_dev, int64_t* out_dev, void* stream)
+{
+    if (!c || !out_dev || what <= 0 || what > (OCT_OBS_W2 | OCT_OBS_CH | OCT_OBS_CS)) return OCT_EINVAL;
+    const bool need_snap = (what & (OCT_OBS_CH | OCT_OBS_CS)) != 0;
+    if (need_snap && (!snapshot_dev || (reinterpret_cast<uintptr_t>(snapshot_dev) & 15u))) return OCT_EINVAL;
+    if ((what & OCT_OBS_CH) && !snapshot_anchor_dev) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 16 * sizeof(int64_t), st));
+    int rc = OCT_OK;
+    if (what & (OCT_OBS_W2 | OCT_OBS_CH)) rc = launch_anchor(c, c->lat, c->anchorA(), st);
+    if (rc) return rc;
+    if (what & OCT_OBS_CH) rc = launch_anchor(c, static_cast<const uint32_t*>(snapshot_dev), c->anchorB(), st);
+    if (rc) return rc;
+    RowsParams rp{};
+    rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
+    rp.anchorA = c->anchorA(); rp.anchorB = c->anchorB(); rp.countersA = c->counters();
+    rp.snapB = reinterpret_cast<const long long*>(snapshot_anchor_dev);
+    rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
+    launch_rows(what, rp, c->L >> 2, st);
+    c->launches++;
+    OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_fetch(oct_ctx* c, const void* src_dev, void* dst_host, size_t bytes, void* stream)
+{
+    if (!c || !src_dev || !dst_host) return OCT_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    OCT_CUDA(c, cudaMemcpyAsync(dst_host, src_dev, bytes, cudaMemcpyDeviceToHost, st));
+    OCT_CUDA(c, cudaStreamSynchronize(st));
     return OCT_OK;
 }
 

@@ -40,6 +40,22 @@ struct SweepParams {
     PhiloxRoundKeys rk;
 };
 
+// Several lattices of one size in one launch (oct_sweep_batch; the paper's curves are ensemble means over n = 20 ... 4367
+// independent runs): blockIdx.y picks the member, which brings its own lattice, counters,
+// seed and clock.  Everything else (size, scheme, rates) is common and sits in `common`.
+constexpr int kMaxBatch = 64;
+struct BatchMember {
+    uint32_t* lat;
+    unsigned long long* counters;
+    uint32_t seed_lo, seed_hi;
+    uint32_t t;
+    uint32_t pad;
+};
+struct SweepBatchParams {
+    SweepParams common;             // lat, counters, t and rk are ignored
+    BatchMember m[kMaxBatch];
+};
+
 template <int LOG2D, int TCX, int TCY, int WPD_>
 struct SweepShape {
     static constexpr int D = 1 << LOG2D;

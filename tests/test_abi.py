@@ -41,7 +41,14 @@ def test_scheme_checks_match_the_header():
         assert ok(cfg.L, cfg.scheme), cfg.name
     for code in wl.ALL_SCHEMES(5):
         assert ok(128, code)
-    assert not ok(128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7))            # L < 2D
+    assert not ok(128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7))            # L < 2D: no room for a 2D x 2D tile
+    # the dead-border layers tile with D x D: a single tile (L = D) is valid there, as in the oracle
+    import oracle
+    for dev in (wl.DEV_DTR, wl.DEV_DT, wl.DEV_DB, wl.DEV_CDB, wl.DEV_DBH):
+        for L, lD in ((64, 6), (128, 6), (32, 5), (128, 7), (256, 8), (64, 7)):
+            code = wl.scheme_code(dev, wl.BLK_DB, lD)
+            assert ok(L, code) == (oracle.lib().orc_check_scheme(L, code) == 0), (dev, L, lD)
+    assert ok(64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6)) and not ok(64, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6))
     assert not ok(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6, 0, 0))      # DT needs TC >= 1,1 (:182)
     assert not ok(256, wl.scheme_code(5, 0, 6)) and not ok(256, wl.scheme_code(0, 4, 6))
     assert ok(256, wl.scheme_code(wl.DEV_DBH, wl.BLK_DB, 6))
@@ -59,6 +66,10 @@ def test_null_and_invalid_arguments_do_not_crash():
     assert lib.oct_create(C.byref(h), 256, 1, 0, None, None, None) == binding.OCT_EINVAL
     assert lib.oct_create(C.byref(h), 256, 1, 7, 16, 16, None) == binding.OCT_EINVAL
     assert lib.oct_sweep(None, 1, 1.0, 0.0, 0, None) == binding.OCT_EINVAL
+    assert lib.oct_sweep_batch(None, 1, 1, 1.0, 0.0, 0, None) == binding.OCT_EINVAL
+    two = (C.c_void_p * 2)(None, None)
+    assert lib.oct_sweep_batch(two, 2, 1, 1.0, 0.0, 0, None) == binding.OCT_EINVAL
+    assert lib.oct_sweep_batch(two, 0, 1, 1.0, 0.0, 0, None) == binding.OCT_EINVAL
     assert lib.oct_destroy(None) == binding.OCT_EINVAL
     assert lib.oct_strerror(0) == b"ok" and lib.oct_strerror(-1) == b"invalid argument"
     assert lib.oct_last_error(None) == b""

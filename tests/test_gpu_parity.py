@@ -60,6 +60,15 @@ SMALL = [
     (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 6), 1.0, 0.0, 8),
     (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DT, 6), 1.0, 0.0, 8),
     (64, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5), 1.0, 0.0, 16),               # L = 2D: a single tile
+    (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 12),                # L = D: a single dead-border tile
+    (64, wl.scheme_code(wl.DEV_CDB, wl.BLK_DT, 6), 0.7, 0.3, 8),
+    (32, wl.scheme_code(wl.DEV_DBH, wl.BLK_DB, 5), 0.9, 0.1, 12),
+    (128, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 7), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8), 0.8, 0.2, 4),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 0.9, 0.1, 5),         # two domains per warp, delayed borders
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6, 2, 2), 0.6, 0.4, 5),
+    (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 6),          # ... of which one has no domain (4 tiles, odd split)
+    (64, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 5), 0.5, 0.5, 10),               # D = 32 TC=1,1: half-warp groups, one tile
     (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 5), 0.5, 0.5, 16),
     (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 0, 0), 1.0, 0.0, 8),
     (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 2, 2), 0.8, 0.2, 8),
@@ -257,3 +266,59 @@ def test_invalid_calls_are_rejected_without_side_effects():
         assert e.value.code == binding.OCT_EINVAL
     assert (sim.oct_export() == before).all() and sim.oct_mcs() == 0
     sim.close()
+
+
+def test_batch_members_equal_their_single_runs_and_the_oracle():
+    """oct_sweep_batch (many lattices of one size per launch, PAPER.md:200/:232 ensembles): every member ends bit-identical
+    to the oracle run with that member's seed -- also with unequal clocks, for a dead-border layer, for two domains per
+    warp, and for a shape that has no batch kernel (members run one after the other)."""
+    cases = [(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 1.0, 0.0, 5, 5),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 0.8, 0.2, 3, 3),
+             (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 5), 0.7, 0.3, 4, 70),      # more members than one launch holds
+             (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 4, 3),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 3, 4),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 1.0, 0.0, 2, 3)]
+    for L, code, p, q, n, members in cases:
+        seeds = [500 + 7 * i for i in range(members)]
+        sims = [binding.Sim(L, sd) for sd in seeds]
+        sims[0].oct_sweep(2, p, q, code)                               # member 0 starts two sweeps ahead
+        binding.oct_sweep_batch(sims, n, p, q, code)
+        for i in sorted(set([0, 1, members // 2, members - 1])):
+            orc = Oracle(L, seeds[i])
+            orc.sweep(n + (2 if i == 0 else 0), p, q, code)
+            compare_state(sims[i], orc, check_heights=False)
+            orc.close()
+        for s_ in sims:
+            s_.close()
+
+
+@pytest.mark.parametrize("L", [16, 64, 1024, 4096])
+def test_one_pass_observables_equal_the_three_separate_calls_and_the_oracle(L):
+    """oct_observe: any combination of the W^2, C_h and C_s sums in ONE pass over lattice + snapshot."""
+    h, h2 = sf.separable_surface(L, 5, 40), sf.separable_surface(L, 105, -3)
+    lat = torch.from_numpy(sf.pack_heights(h).view(np.int32).reshape(-1)).cuda()
+    sim = binding.Sim(L, 0, lattice=lat)
+    sim.oct_set_state(11, 40, 9)
+    snap = torch.from_numpy(sf.pack_heights(h2).view(np.int32).reshape(-1)).cuda()
+    anchor = torch.tensor([-3, 4], dtype=torch.int64, device="cuda")
+    orc = Oracle(L, 0); orc.set_lattice(sf.pack_heights(h), h00=40, net=9)
+    osn = Oracle(L, 0); osn.set_lattice(sf.pack_heights(h2), h00=-3, net=4)
+    want = {1: orc.sums(), 2: orc.autocorr_sums(osn), 4: orc.slope_autocorr_sums(osn)}
+    sl = {1: slice(0, 4), 2: slice(4, 9), 4: slice(9, 15)}
+    for what in range(1, 8):
+        out = [int(v) for v in sim.oct_observe(what, snap, anchor).cpu().numpy()]
+        for bit in (1, 2, 4):
+            got = tuple(out[sl[bit]])
+            assert got == (want[bit] if what & bit else (0,) * len(want[bit])), (L, what, bit)
+        assert out[15] == 0
+    assert tuple(int(v) for v in sim.oct_width2().cpu().numpy()) == want[1]
+    assert tuple(int(v) for v in sim.oct_autocorr(snap, anchor).cpu().numpy()) == want[2]
+    assert tuple(int(v) for v in sim.oct_slope_autocorr(snap).cpu().numpy()) == want[4]
+    with pytest.raises(binding.OctError):
+        sim.oct_observe(2, None, None)
+    with pytest.raises(binding.OctError):
+        sim.oct_observe(8, snap, anchor)
+    host = np.zeros(16, dtype=np.int64)
+    sim.oct_fetch(sim.oct_observe(7, snap, anchor), host.ctypes.data, 128)
+    assert tuple(host[:4]) == want[1] and tuple(host[9:15]) == want[4]
+    sim.close(); orc.close(); osn.close()

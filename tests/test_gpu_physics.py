@@ -23,7 +23,7 @@ torch = pytest.importorskip("torch")
 def late_cs(dev):
     out = run.main(["--L", "2048", "--mcs", "3100", "--snap", "100", "--log2D", "6", "--dev", str(dev),
                     "--blk", str(wl.BLK_DT), "--seeds", "8", "--per-decade", "4"])
-    late = [r for r in out["ensemble"] if r["t"] >= 1000 and "c_s" in r]
+    late = [r for r in out["ensemble"] if r["sweeps"] >= 1000 and "c_s" in r]
     assert len(late) >= 5
     mean = sum(r["c_s"] for r in late) / len(late)
     sem = math.sqrt(sum(r["c_s_sem"] ** 2 for r in late) / len(late))          # typical per-point standard error
@@ -46,7 +46,7 @@ def test_finer_block_layer_decomposition_gives_a_smaller_roughness_prefactor():
     def w2_at(tc, t_probe=(32, 100, 316)):
         out = run.main(["--L", "4096", "--mcs", "316", "--log2D", "7", "--tcx", str(tc), "--tcy", str(tc),
                         "--seeds", "8", "--per-decade", "4"])
-        rows = {r["t"]: r for r in out["ensemble"]}
+        rows = {r["sweeps"]: r for r in out["ensemble"]}
         return [(rows[t]["w2"], rows[t]["w2_sem"]) for t in t_probe]
     fine, coarse = w2_at(1), w2_at(2)
     for k, ((wf, sf), (wc, sc)) in enumerate(zip(fine, coarse)):

@@ -31,4 +31,20 @@ def test_ensemble_mean_and_standard_error():
     assert e[0]["w2"] == 2.0 and e[0]["w2_sem"] == pytest.approx(1.0)        # sqrt(((1)^2+(1)^2)/(2*1))
     assert e[1]["w2"] == 5.0 and e[1]["mean_h_sem"] == pytest.approx(1.0)
     assert e[1]["beta_eff"] == pytest.approx(math.log(5.0 / 2.0) / math.log(10.0) / 2)
+    # propagated 1-sigma error: sqrt((1/5)^2 + (1/2)^2) / ln 10 / 2, and the spread of the per-run exponents
+    assert e[1]["beta_eff_err"] == pytest.approx(math.sqrt(0.2 ** 2 + 0.5 ** 2) / math.log(10.0) / 2)
+    b = [math.log(4.0) / math.log(10.0) / 2, math.log(2.0) / math.log(10.0) / 2]
+    assert e[1]["beta_eff_sem"] == pytest.approx(abs(b[0] - b[1]) / 2)
     assert "c_h" not in e[0]
+
+
+def test_aging_exponent_and_its_error_use_t_over_s():
+    # C_h = 7 (t/s)^(-1.21) (lambda_h/z of PAPER.md:100-104 is about 1.21 for KPZ): recovered between any two points
+    s = 100.0
+    f = lambda t: 7.0 * (t / s) ** -1.21
+    runs = [[{"t": 200.0, "w2": 1.0, "c_h": f(200.0) * k}, {"t": 400.0, "w2": 2.0, "c_h": f(400.0) * k}] for k in (0.9, 1.1)]
+    e = run.ensemble_mean(runs, snap_t=s)
+    assert e[1]["lambda_h_over_z_eff"] == pytest.approx(1.21)
+    rel = 0.1 / math.sqrt(2) * math.sqrt(2)          # each point: values 0.9x and 1.1x -> sem = 0.1 x
+    assert e[1]["lambda_h_over_z_eff_err"] == pytest.approx(math.sqrt(2) * rel / math.log(2.0))
+    assert run.eff_exponent_err(1.0, 0.1, 10, 0.0, 0.1, 5) is None
