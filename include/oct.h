@@ -102,7 +102,7 @@ int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* st
 
 /* The same n_mcs sweeps on n independent simulations of ONE lattice size at once (ensembles: the paper's curves are
  * means over n = 20 ... 4367 runs, many at L <= 2^13): every kernel launch covers the
- * domains of all members (grid = domains x members, at most 64 members per launch), so small lattices fill the
+ * domains of all members (grid = domains x members, at most 256 members per launch), so small lattices fill the
  * GPU.  Each member keeps its own lattice, counters, seed and clock; its result is bit-identical to what
  * oct_sweep on that handle alone would give.  Shapes without a many-lattices kernel (D > 64, bit-packed kernel)
  * run the members one after the other.  The kernel option of handle 0 applies.

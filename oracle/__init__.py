@@ -21,13 +21,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oct_oracle.c")
 _LIB = os.path.join(_HERE, "liboct_oracle.so")
 
-# scheme encoding of include/oct.h (restated, not shared): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16
+# scheme encoding of include/oct.h (restated, not shared): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 | ka<<21 | w<<23
 DEV_DTR, DEV_DT, DEV_DB, DEV_CDB, DEV_DBH = 0, 1, 2, 3, 4
 BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR = 0, 1, 2, 3
 
 
-def scheme(dev: int, blk: int, log2D: int, tcx: int = 1, tcy: int = 1) -> int:
-    return dev | (blk << 4) | (tcx << 8) | (tcy << 12) | (log2D << 16)
+def scheme(dev: int, blk: int, log2D: int, tcx: int = 1, tcy: int = 1, ka: int = 0, w: int = 0) -> int:
+    """ka: t_async = 2^-ka MCS; w: explicit dead-border width (0 = the scheme's own) -- dead-border device layers only."""
+    return dev | (blk << 4) | (tcx << 8) | (tcy << 12) | (log2D << 16) | (ka << 21) | (w << 23)
 
 
 def build(force: bool = False) -> str:

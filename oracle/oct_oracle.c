@@ -9,7 +9,7 @@
  * What each part follows (PAPER.md line : section):
  *   - update rule                      Eq. (1) :27-34, Fig. 1 caption :50, :52, :140   -> orc_attempt
  *   - true random-sequential dynamics  :15/:44, 1 MCS = L^2 attempts :106               -> orc_sweep_rs
- *   - device-layer DD: DB/cDB          Sec. 3.0.1 :133-140, :166; t_async = 1/2 :204-206 -> orc_sweep_dd
+ *   - device-layer DD: DB/cDB          Sec. 3.0.1 :133-140, :166; t_async = 1/2^k :204-206, border width :202 -> orc_sweep_dd
  *                      DT, DTr         Sec. 3.0.2 :142-146, Sec. 3.0.3 :148-150          -> orc_sweep_dd
  *   - block-layer single-hit DB / DT   Sec. 3.1 :168-174; DT with moving origin (DTr) :234 -> domain_sweep
  *   - roughness W^2, autocorr C_h      Eq. (3) :61, Eq. (6) :92-98                       -> orc_sums, orc_autocorr_sums
@@ -240,7 +240,9 @@ int orc_sweep_rs(orc_state *s, uint64_t n_mcs, double p, double q)
 
 /* ------------------------------------------------------------------------------- DD schemes */
 
-/* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16   (include/oct.h) */
+/* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 | ka<<21 | w<<23   (include/oct.h)
+ * ka (dead-border layers only): t_async = 2^-ka MCS, i.e. 2^ka asynchronous intervals per sweep (:204-206, R27);
+ * w  (dead-border layers only): dead-border width in sites, 0 = the scheme's own (DB 5, cDB 1; :166, :196-202, R22/R28). */
 enum { DEV_DTR = 0, DEV_DT = 1, DEV_DB = 2, DEV_CDB = 3, DEV_DBH = 4 };
 enum { BLK_DB_AUTO = 0, BLK_DB_DELAYED = 1, BLK_DT = 2, BLK_DTR = 3 };
 
@@ -372,9 +374,12 @@ static void lex_perm4(uint32_t idx, uint32_t perm[4])
 int orc_check_scheme(uint32_t L, uint32_t scheme)
 {
     const uint32_t dev = scheme & 15u, blk = (scheme >> 4) & 15u, tcx = (scheme >> 8) & 15u,
-                   tcy = (scheme >> 12) & 15u, lD = (scheme >> 16) & 31u;
-    if (dev > 4 || blk > 3 || lD < 3 || lD > 12) return -1;
+                   tcy = (scheme >> 12) & 15u, lD = (scheme >> 16) & 31u, ka = (scheme >> 21) & 3u, w = (scheme >> 23) & 7u;
+    if ((scheme >> 26) != 0 || dev > 4 || blk > 3 || lD < 3 || lD > 12) return -1;
+    if ((ka || w) && dev != DEV_DB && dev != DEV_CDB) return -1;   /* t_async and width belong to the dead-border layers; DBh is DB with ka = 1 */
+    if (ka > 2) return -1;                                          /* the interval index shares the 2-bit set field of the counters (R19) */
     const uint32_t D = 1u << lD, cx = 4u << tcx, cy = 4u << tcy;
+    if (w >= D || ((cx * cy) >> ka) < 4 || ((cx * cy) >> ka) % 4 != 0) return -1;   /* whole Philox calls (4 steps) per interval */
     if (cx > 64 || cy > 64 || cx > D || cy > D) return -1;
     if ((blk == BLK_DT || blk == BLK_DTR) && (tcx < 1 || tcy < 1)) return -1;   /* :182 smallest TC=1,1 for DT */
     if (!is_pow2(L)) return -1;
@@ -388,7 +393,7 @@ int orc_sweep_dd(orc_state *s, uint64_t n_mcs, double p, double q, uint32_t sche
 {
     if (orc_check_scheme(s->L, scheme)) return -1;
     const uint32_t dev = scheme & 15u, blk = (scheme >> 4) & 15u, tcx = (scheme >> 8) & 15u,
-                   tcy = (scheme >> 12) & 15u, lD = (scheme >> 16) & 31u;
+                   tcy = (scheme >> 12) & 15u, lD = (scheme >> 16) & 31u, ka = (scheme >> 21) & 3u, wsel = (scheme >> 23) & 7u;
     const uint32_t D = 1u << lD, cx = 4u << tcx, cy = 4u << tcy, L = s->L, m = L - 1;
     const uint32_t P16 = orc_prob16(p), Q16 = orc_prob16(q);
     const uint32_t key[2] = { (uint32_t)s->seed, (uint32_t)(s->seed >> 32) };
@@ -423,10 +428,10 @@ int orc_sweep_dd(orc_state *s, uint64_t n_mcs, double p, double q, uint32_t sche
             free(dorder);
         } else {
             /* :135 dead border; :166 cDB = origin on the 4x4 word grid, border 1; DB = free origin, border 5.
-             * DBh (:204-206, R27): DB with t_async = 1/2 MCS -- two intervals per sweep, each with
-             * its own origin (global stream c0 = interval) and half of the collective steps. */
-            const uint32_t n_int = dev == DEV_DBH ? 2u : 1u;
-            const uint32_t dead_w = dev == DEV_CDB ? 1u : 5u;
+             * t_async = 1/n_int MCS (:204-206, R27; DBh = DB with two intervals): n_int intervals per sweep, each
+             * with its own origin (global stream c0 = interval) and 1/n_int of the collective steps. */
+            const uint32_t n_int = dev == DEV_DBH ? 2u : (1u << ka);              /* t_async = 1 / n_int MCS (:204-206) */
+            const uint32_t dead_w = wsel ? wsel : (dev == DEV_CDB ? 1u : 5u);     /* :166; explicit width: :202, R28 */
             const uint32_t nt = L / D;
             uint32_t *dorder = (uint32_t *)malloc((size_t)nt * nt * sizeof(uint32_t));
             if (!dorder) return -3;

@@ -222,6 +222,7 @@ struct SweepPlan {
     SchemeFields f;
     SweepLaunch sl;
     uint32_t P16, Q16, ndom, grid, n_launch;
+    bool pdl;                        // link-entry kernels wait for their predecessor themselves (griddepcontrol.wait)
 };
 
 int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
@@ -239,6 +240,7 @@ int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
                        find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B,
                                          f.dev > OCT_DEV_DT, &pl->sl);
     if (!links && !find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &pl->sl)) return OCT_EINVAL;
+    pl->pdl = links;
     const bool tiled = f.dev <= OCT_DEV_DT;
     const uint32_t nt = tiled ? c->L >> (f.log2D + 1) : c->L >> f.log2D;
     pl->ndom = nt * nt;
@@ -257,6 +259,20 @@ int opt_in_smem(oct_ctx* c, const void* fn, int smem)
     OCT_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     if (n_done < 64) done[n_done++] = fn;
     return OCT_OK;
+}
+
+// Launch a sweep kernel with programmatic stream serialisation: the kernel may be scheduled while its predecessor in
+// the stream drains; it waits for the predecessor's completion (griddepcontrol.wait) before its first global access.
+template <class PARAMS>
+cudaError_t launch_sweep(void (*kern)(const PARAMS), dim3 grid, int threads, int smem, cudaStream_t st, const PARAMS& p, bool pdl)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = dim3((unsigned)threads); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1u : 0u;
+    return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
 void fill_common(SweepParams& sp, const oct_ctx* c, const SweepPlan& pl)
@@ -287,7 +303,7 @@ int oct_sweep(oct_ctx* c, uint64_t n_mcs, double p, double q, int scheme, void* 
         sp.t = static_cast<uint32_t>(c->t);
         for (uint32_t si = 0; si < pl.n_launch; ++si) {   // :144 sync = kernel boundary after each set
             sp.si = si;
-            pl.sl.kern<<<pl.grid, pl.sl.threads, pl.sl.smem, st>>>(sp);
+            OCT_CUDA(c, launch_sweep(pl.sl.kern, dim3(pl.grid), pl.sl.threads, pl.sl.smem, st, sp, pl.pdl));
             c->launches++;
         }
         OCT_CUDA(c, cudaGetLastError());   // on failure the clock stays at the sweeps completed so far (oct_mcs)
@@ -333,7 +349,7 @@ int oct_sweep_batch(oct_ctx* const* cs, uint32_t n, uint64_t n_mcs, double p, do
             }
             for (uint32_t si = 0; si < pl.n_launch; ++si) {
                 bp.common.si = si;
-                pl.sl.kern_batch<<<dim3(pl.grid, nb), pl.sl.threads, pl.sl.smem, st>>>(bp);
+                OCT_CUDA(c0, launch_sweep(pl.sl.kern_batch, dim3(pl.grid, nb), pl.sl.threads, pl.sl.smem, st, bp, pl.pdl));
                 c0->launches++;
             }
         }

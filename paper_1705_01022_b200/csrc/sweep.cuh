@@ -43,7 +43,7 @@ struct SweepParams {
 // Several lattices of one size in one launch (oct_sweep_batch; the paper's curves are ensemble means over n = 20 ... 4367
 // independent runs): blockIdx.y picks the member, which brings its own lattice, counters,
 // seed and clock.  Everything else (size, scheme, rates) is common and sits in `common`.
-constexpr int kMaxBatch = 64;
+constexpr int kMaxBatch = 256;
 struct BatchMember {
     uint32_t* lat;
     unsigned long long* counters;

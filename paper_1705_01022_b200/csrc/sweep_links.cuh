@@ -474,6 +474,13 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     auto kept = [&](uint32_t iw, uint32_t jw) -> bool { return !DEAD || (iw < ncol && jw < nrow); };
     auto word_ptr = [&](uint32_t iw, uint32_t jw) -> uint32_t* { return lat + (size_t)((wy0 + jw) & LWm) * LW + ((wx0 + iw) & LWm); };
 
+    // Programmatic dependent launch: the launches of one MCS depend on each other (kernel boundary = the device-wide
+    // synchronisation of :144), but everything above touches no global memory, so the next launch's CTAs may take
+    // their SM slots while this grid drains and wait HERE for its completion (hides the launch ramp: matters for
+    // small lattices / ensembles, where a launch lasts ~20 us).
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+
     // ---- a2: stage-in (:164): packed words -> link entries -------------------------------------
     int net = 0;                                     // deposits - removals, from the x-moments (see x_moment)
     if constexpr (SH::FAST_17 && G == 16) {

@@ -274,7 +274,7 @@ def test_batch_members_equal_their_single_runs_and_the_oracle():
     warp, and for a shape that has no batch kernel (members run one after the other)."""
     cases = [(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 1.0, 0.0, 5, 5),
              (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 0.8, 0.2, 3, 3),
-             (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 5), 0.7, 0.3, 4, 70),      # more members than one launch holds
+             (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 5), 0.7, 0.3, 3, 260),     # more members than one launch holds (256)
              (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 4, 3),
              (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 3, 4),
              (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 1.0, 0.0, 2, 3)]

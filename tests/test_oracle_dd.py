@@ -248,6 +248,77 @@ def test_dead_border_half_sweep_intervals():
     o.close(); o_db.close()
 
 
+def _fit_origin(part, L, D, nt):
+    """the ONE tiling origin (Ox, Oy) that puts every traced attempt of tile `dom` into that tile"""
+    found = []
+    for axis, col in (("x", lambda d: d % nt), ("y", lambda d: d // nt)):
+        for O in range(L):
+            l = (part[axis].astype(np.int64) - O) % L
+            if ((l // D) == col(part["dom"])).all():
+                found.append(O)
+                break
+        else:
+            raise AssertionError(f"no {axis} origin fits")
+    return tuple(found)
+
+
+@pytest.mark.parametrize("dev,ka,w", [(DEV_DB, 2, 0), (DEV_DB, 1, 0), (DEV_DB, 0, 1), (DEV_DB, 2, 1), (DEV_DB, 1, 3), (DEV_CDB, 1, 0), (DEV_CDB, 0, 2)])
+def test_general_t_async_and_border_width(dev, ka, w):
+    """DB / cDB with t_async = 2^-ka MCS and an explicit border width (R27/R28), from the attempt trace:
+    2^ka intervals per sweep, each with its own origin (free for DB, on the 4-site grid for cDB) and 1/2^ka of the
+    collective steps; an attempt is discarded iff it falls into the rim of the stated width; L^2 attempts per sweep."""
+    L, seed, D, cx, cy = 128, 31, 32, 8, 8
+    width = w if w else (1 if dev == DEV_CDB else 5)
+    n_int = 1 << ka
+    code = scheme(dev, BLK_DB, 5, 1, 1, ka, w)
+    o, tr = run_traced(L, seed, code, 2, 0.8, 0.2)
+    assert len(tr) == 2 * L * L
+    nt, per = L // D, cx * cy // n_int
+    seen = set()
+    for t in range(2):
+        rec = tr[tr["t"] == t]
+        for iv in range(n_int):
+            part = rec[(rec["k"] >= iv * per) & (rec["k"] < (iv + 1) * per)]
+            assert len(part) == L * L // n_int and (part["set"] == iv).all()
+            Ox, Oy = _fit_origin(part, L, D, nt)
+            if dev == DEV_CDB:
+                assert Ox % 4 == 0 and Oy % 4 == 0
+            seen.add((Ox % 4, Oy % 4))
+            lx, ly = (part["x"].astype(np.int64) - Ox) % L % D, (part["y"].astype(np.int64) - Oy) % L % D
+            assert ((part["result"] == 2) == ((lx >= D - width) | (ly >= D - width))).all()
+            for dom in (0, nt * nt - 1):
+                assert (part["dom"] == dom).sum() == D * D // n_int
+            if iv == 0:
+                assert (Ox, Oy) == oracle.mcs_control(seed, t, L, dev)[:2]              # interval 0 = the plain draw (c0 = 0)
+    if dev == DEV_DB and n_int * 2 >= 4:
+        assert len(seen) > 1                                                            # free origin: not on a coarse grid
+    # discarded fraction = border fraction N_border / N of Eq. (9)
+    frac = (tr["result"] == 2).mean()
+    assert abs(frac - (1 - ((D - width) / D) ** 2)) < 0.01
+    o.close()
+
+
+def test_t_async_and_width_reduce_to_the_named_schemes():
+    L, seed = 128, 5
+    runs = {}
+    for name, code in (("DBh", scheme(DEV_DBH, BLK_DB, 5)), ("DB ka=1", scheme(DEV_DB, BLK_DB, 5, 1, 1, 1, 0)),
+                       ("DB", scheme(DEV_DB, BLK_DB, 5)), ("DB w=5", scheme(DEV_DB, BLK_DB, 5, 1, 1, 0, 5)),
+                       ("cDB", scheme(DEV_CDB, BLK_DT, 5)), ("cDB w=1", scheme(DEV_CDB, BLK_DT, 5, 1, 1, 0, 1)),
+                       ("DB w=1", scheme(DEV_DB, BLK_DB, 5, 1, 1, 0, 1)), ("DB ka=2", scheme(DEV_DB, BLK_DB, 5, 1, 1, 2, 0))):
+        o = Oracle(L, seed)
+        o.sweep(6, 0.7, 0.3, code)
+        runs[name] = (o.lattice.copy(), o.net, o.h00)
+        o.close()
+    same = lambda a, b: (runs[a][0] == runs[b][0]).all() and runs[a][1:] == runs[b][1:]     # noqa: E731
+    assert same("DBh", "DB ka=1") and same("DB", "DB w=5") and same("cDB", "cDB w=1")
+    assert not same("DB", "DB w=1") and not same("DB", "DB ka=2") and not same("DB ka=1", "DB ka=2")
+    # the fields belong to the dead-border layers only; at most four intervals; whole Philox calls per interval
+    chk = oracle.lib().orc_check_scheme
+    assert chk(L, scheme(DEV_DTR, BLK_DB, 5, 1, 1, 1, 0)) != 0 and chk(L, scheme(DEV_DT, BLK_DB, 5, 1, 1, 0, 1)) != 0
+    assert chk(L, scheme(DEV_DBH, BLK_DB, 5, 1, 1, 1, 0)) != 0 and chk(L, scheme(DEV_DB, BLK_DB, 5, 1, 1, 3, 0)) != 0
+    assert chk(L, scheme(DEV_DB, BLK_DB, 5, 0, 0, 2, 0)) == 0 and chk(L, scheme(DEV_DB, BLK_DB, 5, 1, 1, 2, 7)) == 0
+
+
 def test_origin_and_permutation_statistics():
     L = 1024
     ox, oy, perms = [], [], []
@@ -290,6 +361,8 @@ ORDER_CASES = [
     (scheme(DEV_DTR, BLK_DB, 5, 0, 0), 0.5, 0.5), (scheme(DEV_DTR, BLK_DB, 6, 3, 1), 1.0, 0.0),
     (scheme(DEV_DTR, BLK_DTR, 5), 0.6, 0.4), (scheme(DEV_DTR, BLK_DTR, 5, 2, 1), 1.0, 0.0),
     (scheme(DEV_DBH, BLK_DB, 5), 0.7, 0.3), (scheme(DEV_DBH, BLK_DT, 5), 1.0, 0.0),
+    (scheme(DEV_DB, BLK_DB, 5, 1, 1, 2, 0), 0.7, 0.3), (scheme(DEV_DB, BLK_DB, 5, 1, 1, 0, 1), 0.6, 0.4),      # t_async = 1/4; width 1, free origin
+    (scheme(DEV_DB, BLK_DT, 5, 1, 1, 1, 2), 1.0, 0.0), (scheme(DEV_CDB, BLK_DB, 5, 1, 1, 2, 3), 0.9, 0.1),
 ]
 
 

@@ -211,6 +211,8 @@ CASES = [
     (scheme(DEV_DTR, 3, 5), 0.7, 0.3),            # block-layer DTr
     (scheme(DEV_DB, 3, 5, 2, 1), 1.0, 0.0),
     (scheme(4, BLK_DB, 5), 0.8, 0.2),             # DB with t_async = 1/2
+    (scheme(DEV_DB, BLK_DB, 5, 1, 1, 2, 1), 0.8, 0.2),   # t_async = 1/4, border width 1 with a free origin (:202-206)
+    (scheme(DEV_CDB, BLK_DT, 5, 1, 1, 1, 3), 1.0, 0.0),
 ]
 
 
