@@ -50,7 +50,7 @@ enum {
     OCT_INIT_FROM_DEVICE = 2    /* the caller already filled lattice_dev (canonical words)          */
 };
 
-/* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16            (notation of Sec. 3.1.1 :176-182)
+/* scheme = dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 | ka<<21 | w<<23      (notation of Sec. 3.1.1 :176-182)
  *   dev  (device layer, Sec. 3 :129-150):  0 DTr  double tiling with random origin   (:148-150)
  *                                          1 DT   double tiling, fixed origin         (:142-146)
  *                                          2 DB   dead border, free origin, width 5   (:133-140, :166)
@@ -65,9 +65,15 @@ enum {
  *                                          2 DT   one random quadrant of every cell per step (:170)
  *                                          3 DTr  DT whose cell origin also moves every step ("DTrDTr", :234, R26)
  *   tcx,tcy: log2 of the thread-cell edge in words of 4 sites, "TC=tcx,tcy" (:180); cell = 4<<tc sites
- *   log2D  : log2 of the device-layer domain edge D in sites (the sub-tile one worker sweeps)       */
+ *   log2D  : log2 of the device-layer domain edge D in sites (the sub-tile one worker sweeps)
+ *   ka     : dead-border layers DB / cDB only: t_async = 2^-ka MCS, ka = 0, 1, 2 -- one sweep is 2^ka asynchronous
+ *            intervals, each with its own origin and 1/2^ka of the collective steps (:204-206, R27; DBh == DB with ka = 1)
+ *   w      : DB / cDB only: dead-border width in sites, 1..7; 0 = the scheme's own (DB 5, cDB 1).  DB with w = 1 is the
+ *            "DB with a border-width of one lattice site" and a free origin of :208; the paper's bit-coded kernel needs 5
+ *            there because tiles share 4x4-site words (:166) -- here words shared by two tiles are written back bit-wise  */
 #define OCT_SCHEME(dev, blk, tcx, tcy, log2D) \
     ((dev) | ((blk) << 4) | ((tcx) << 8) | ((tcy) << 12) | ((log2D) << 16))
+#define OCT_SCHEME_DB(dev, blk, tcx, tcy, log2D, ka, w) (OCT_SCHEME(dev, blk, tcx, tcy, log2D) | ((ka) << 21) | ((w) << 23))
 enum { OCT_DEV_DTR = 0, OCT_DEV_DT = 1, OCT_DEV_DB = 2, OCT_DEV_CDB = 3, OCT_DEV_DBH = 4 };
 enum { OCT_BLK_DB = 0, OCT_BLK_DB_DELAYED = 1, OCT_BLK_DT = 2, OCT_BLK_DTR = 3 };
 
@@ -90,7 +96,7 @@ int oct_set_state(oct_ctx*, uint64_t t_mcs, int64_t h00, int64_t net, void* stre
 /* n_mcs sweeps of the whole lattice (1 MCS = L^2 update attempts, :106) under DD scheme `scheme`,
  * deposition probability p at local minima and removal probability q at local maxima (Eq. (1)
  * :27-34; p,q in [0,1], quantised to 1/65536, R18).  DTr/DT: 4 kernel launches per MCS, one per domain
- * set, in the permutation drawn for that MCS (:144); DB/cDB: 1 launch per MCS (DBh: 2), and one such sweep
+ * set, in the permutation drawn for that MCS (:144); DB/cDB: 2^ka launches per sweep (DBh: 2), and one such sweep
  * lasts (1 - N_border/N) MCS of physical time (Eq. (9) :137, R9; see oct_time_per_sweep).
  * oct_sweep(a) followed by oct_sweep(b) equals oct_sweep(a+b).
  * Errors (nothing is enqueued): EINVAL for p,q outside [0,1], unknown dev/blk, cell larger than the
@@ -179,7 +185,7 @@ int oct_launch_count(const oct_ctx*, uint64_t* n_out);
 double oct_w2_from_sums(uint32_t L, int64_t S1, int64_t S2);                    /* (N*S2 - S1^2)/N^2  */
 double oct_c_from_sums(uint32_t L, int64_t St, int64_t Ss, int64_t Sts);        /* (N*Sts - St*Ss)/N^2 */
 double oct_cs_from_sums(uint64_t M, int64_t n11, int64_t n1t, int64_t n1s);     /* (M*n11 - n1t*n1s)/M^2 */
-double oct_time_per_sweep(uint32_t L, int scheme);   /* 1 for DT/DTr; (1 - N_border/N) for DB/cDB (R9) */
+double oct_time_per_sweep(uint32_t L, int scheme);   /* 1 for DT/DTr; (1 - N_border/N) = ((D-w)/D)^2 for DB/cDB/DBh (R9) */
 int    oct_scheme_supported(uint32_t L, int scheme); /* OCT_OK or OCT_EINVAL, same checks as oct_sweep */
 
 #ifdef __cplusplus

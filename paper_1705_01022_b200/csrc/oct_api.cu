@@ -83,22 +83,31 @@ bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, bool dea
     }
 }
 
-struct SchemeFields { uint32_t dev, blk, tcx, tcy, log2D; };
+struct SchemeFields {
+    uint32_t dev, blk, tcx, tcy, log2D, ka, w;
+    // dead-border layers: intervals per sweep as a power of two (DBh = DB with two) and the border width in sites
+    uint32_t ka_eff() const { return dev == OCT_DEV_DBH ? 1u : ka; }
+    uint32_t width() const { return w ? w : (dev == OCT_DEV_CDB ? 1u : 5u); }
+};
 
 SchemeFields split_scheme(int scheme)
 {
     const uint32_t s = static_cast<uint32_t>(scheme);
-    return {s & 15u, (s >> 4) & 15u, (s >> 8) & 15u, (s >> 12) & 15u, (s >> 16) & 31u};
+    return {s & 15u, (s >> 4) & 15u, (s >> 8) & 15u, (s >> 12) & 15u, (s >> 16) & 31u, (s >> 21) & 3u, (s >> 23) & 7u};
 }
 
 int check_scheme(uint32_t L, int scheme)
 {
     if (scheme < 0 || !valid_L(L)) return OCT_EINVAL;
     const SchemeFields f = split_scheme(scheme);
-    if ((static_cast<uint32_t>(scheme) >> 21) != 0) return OCT_EINVAL;
+    if ((static_cast<uint32_t>(scheme) >> 26) != 0) return OCT_EINVAL;
     if (f.dev > 4 || f.blk > 3) return OCT_EINVAL;
     if (f.log2D < 5 || f.log2D > 8) return OCT_EINVAL;
     const uint32_t D = 1u << f.log2D, cx = 4u << f.tcx, cy = 4u << f.tcy;
+    // t_async and border width belong to DB / cDB (DBh is DB with ka = 1); at most four intervals (they share the 2-bit
+    // set field of the counters, R19), each made of whole Philox calls (4 steps)
+    if ((f.ka || f.w) && f.dev != OCT_DEV_DB && f.dev != OCT_DEV_CDB) return OCT_EINVAL;
+    if (f.ka > 2 || f.w >= D || ((cx * cy) >> f.ka) < 4 || ((cx * cy) >> f.ka) % 4 != 0) return OCT_EINVAL;
     if (cx > D || cy > D || cx > 64 || cy > 64) return OCT_EINVAL;
     const bool blk_dt = f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR;
     if (blk_dt && (f.tcx < 1 || f.tcy < 1)) return OCT_EINVAL;   // :182
@@ -245,7 +254,7 @@ int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
     const uint32_t nt = tiled ? c->L >> (f.log2D + 1) : c->L >> f.log2D;
     pl->ndom = nt * nt;
     pl->grid = (pl->ndom + pl->sl.dpb - 1) / pl->sl.dpb;
-    pl->n_launch = tiled ? 4u : (f.dev == OCT_DEV_DBH ? 2u : 1u);   // :144 one launch per domain set; DBh: two intervals (R27)
+    pl->n_launch = tiled ? 4u : (1u << f.ka_eff());   // :144 one launch per domain set; dead borders: one per interval (R27)
     return OCT_OK;
 }
 
@@ -279,6 +288,7 @@ void fill_common(SweepParams& sp, const oct_ctx* c, const SweepPlan& pl)
 {
     sp.L = c->L; sp.log2L = c->log2L; sp.P16 = pl.P16; sp.Q16 = pl.Q16; sp.dev = pl.f.dev; sp.ndom = pl.ndom;
     sp.dtr_mask = pl.f.blk == OCT_BLK_DTR ? ~0u : 0u;
+    sp.dead_w = pl.f.width(); sp.ka = pl.f.ka_eff();
 }
 
 }  // namespace
@@ -562,7 +572,7 @@ double oct_time_per_sweep(uint32_t L, int scheme)
     if (check_scheme(L, scheme) != OCT_OK) return 0.0;
     const SchemeFields f = split_scheme(scheme);
     if (f.dev <= OCT_DEV_DT) return 1.0;
-    const double D = (double)(1u << f.log2D), w = f.dev == OCT_DEV_CDB ? 1.0 : 5.0;   // DB and DBh: 5
+    const double D = (double)(1u << f.log2D), w = (double)f.width();
     return ((D - w) / D) * ((D - w) / D);   // Eq. (9) :137 with reading R9
 }
 

@@ -32,13 +32,46 @@ struct SweepParams {
     uint32_t L;
     uint32_t log2L;
     uint32_t t;                     // absolute MCS index of this sweep
-    uint32_t si;                    // position of this launch in the set permutation (0..3); DBh: interval 0/1; else 0
+    uint32_t si;                    // position of this launch in the set permutation (0..3); dead-border layers: interval index
     uint32_t P16, Q16;              // acceptance thresholds, accept iff r16 < P16 (R18)
     uint32_t dev;                   // device-layer scheme
     uint32_t ndom;                  // domains in this launch
     uint32_t dtr_mask;              // block-layer DT: 0; block-layer DTr (:234, R26): ~0 (the origin also moves)
+    uint32_t dead_w;                // dead-border layers: border width in sites (DB 5, cDB 1, or the explicit one; :166, :202, R22/R28)
+    uint32_t ka;                    // dead-border layers: t_async = 2^-ka MCS, 2^ka launches (intervals) per sweep (:204-206, R27)
     PhiloxRoundKeys rk;
 };
+
+// Bits of packed window word (iw, jw) that belong to sites of the tile [offx, offx + D) x [offy, offy + D) (window
+// coordinates).  Dead-border tiles with a border narrower than 4 sites and a free origin share words with their
+// neighbours whose other bits the neighbour changes in the same launch (:166 -- the reason for the paper's width 5),
+// so such words are written back bit-wise (two atomics) instead of whole.
+__device__ __forceinline__ uint32_t tile_bits(uint32_t iw, uint32_t jw, uint32_t offx, uint32_t offy, uint32_t D)
+{
+    uint32_t m = 0u;
+#pragma unroll
+    for (uint32_t i = 0; i < 4; ++i) {
+        const uint32_t x = 4u * iw + i;
+        if (x >= offx && x < offx + D) m |= 0x03030303u << (2u * i);
+    }
+#pragma unroll
+    for (uint32_t j = 0; j < 4; ++j) {
+        const uint32_t y = 4u * jw + j;
+        if (!(y >= offy && y < offy + D)) m &= ~(0xFFu << (8u * j));
+    }
+    return m;
+}
+
+// write back one window word of a dead-border tile: whole if it holds only this tile's sites (or the border is wide
+// enough that foreign bits cannot change, dead_w >= 4), else only this tile's bits
+__device__ __forceinline__ void store_tile_word(uint32_t* ptr, uint32_t word, uint32_t iw, uint32_t jw, uint32_t offx, uint32_t offy,
+                                                uint32_t D, uint32_t dead_w)
+{
+    const uint32_t m = dead_w >= 4u ? 0xFFFFFFFFu : tile_bits(iw, jw, offx, offy, D);
+    if (m == 0xFFFFFFFFu) { *ptr = word; return; }
+    atomicAnd(ptr, word | ~m);
+    atomicOr(ptr, word & m);
+}
 
 // Several lattices of one size in one launch (oct_sweep_batch; the paper's curves are ensemble means over n = 20 ... 4367
 // independent runs): blockIdx.y picks the member, which brings its own lattice, counters,
@@ -168,11 +201,11 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     if (dom >= P.ndom) return;                       // whole group leaves together (own barrier id)
 
     // ---- a1: per-MCS control from the global stream (:144, :150; R10) --------------------------
-    // DB with t_async = 1/2 (kDevDBh, :204-206, R27): the launch is interval P.si of the sweep, with its own
-    // origin (global stream c0 = interval), half of the collective steps, streams keyed by set = interval
-    const bool half = P.dev == kDevDBh;
+    // dead-border layers with t_async = 2^-ka MCS (:204-206, R27): the launch is interval P.si of the sweep, with its
+    // own origin (global stream c0 = interval), 1/2^ka of the collective steps, streams keyed by set = interval
+    const bool dead = P.dev > kDevDT;
     uint32_t Gw[4];
-    philox4x32_10(half ? P.si : 0u, 0u, kTagGlobal << 30, t, P.rk, Gw);
+    philox4x32_10(dead ? P.si : 0u, 0u, kTagGlobal << 30, t, P.rk, Gw);
     uint32_t gx, gy, set, dead_w;
     if (P.dev <= kDevDT) {
         const uint32_t Ox = P.dev == kDevDTr ? (Gw[0] & Lm) : 0u, Oy = P.dev == kDevDTr ? (Gw[1] & Lm) : 0u;
@@ -185,12 +218,12 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     } else {
         uint32_t Ox = Gw[0] & Lm, Oy = Gw[1] & Lm;
         if (P.dev == kDevCDB) { Ox &= ~3u; Oy &= ~3u; }                 // :166 coarse grid
-        set = half ? P.si : 0u;
+        set = P.si;                                                     // interval index keys the streams (R27)
         const uint32_t lnt = P.log2L - LOG2D;
         const uint32_t I = dom & ((1u << lnt) - 1u), J = dom >> lnt;
         gx = (Ox + (I << LOG2D)) & Lm;
         gy = (Oy + (J << LOG2D)) & Lm;
-        dead_w = P.dev == kDevCDB ? 1u : 5u;                            // :166, R22
+        dead_w = P.dead_w;                                              // :166, R22/R28
     }
     const uint32_t offx = gx & 3u, offy = gy & 3u;
     const uint32_t LW = L >> 2, LWm = LW - 1u, wx0 = gx >> 2, wy0 = gy >> 2;
@@ -217,8 +250,8 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     int net = 0, d00 = 0;
     const uint32_t dead_lim = (uint32_t)D - dead_w;
 
-    const uint32_t k4_begin = half ? P.si * (uint32_t)(SH::NSTEP / 8) : 0u;
-    const uint32_t k4_end = half ? k4_begin + (uint32_t)(SH::NSTEP / 8) : (uint32_t)(SH::NSTEP / 4);
+    const uint32_t k4_per = dead ? (uint32_t)(SH::NSTEP / 4) >> P.ka : (uint32_t)(SH::NSTEP / 4);   // steps of this interval
+    const uint32_t k4_begin = dead ? P.si * k4_per : 0u, k4_end = k4_begin + k4_per;
 #pragma unroll 1
     for (uint32_t k4 = k4_begin; k4 < k4_end; ++k4) {
         uint32_t rw[CPT][4];
@@ -309,7 +342,11 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     const uint32_t ncol = ((offx + (uint32_t)D - dead_w) >> 2) + 1u, nrow = ((offy + (uint32_t)D - dead_w) >> 2) + 1u;
     for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
         const uint32_t j = idx / NW, i = idx - j * NW;
-        if (i < ncol && j < nrow) P.lat[(size_t)((wy0 + j) & LWm) * LW + ((wx0 + i) & LWm)] = S[j * PITCH + i];
+        if (i < ncol && j < nrow) {
+            uint32_t* ptr = P.lat + (size_t)((wy0 + j) & LWm) * LW + ((wx0 + i) & LWm);
+            if (dead) store_tile_word(ptr, S[j * PITCH + i], i, j, offx, offy, (uint32_t)D, dead_w);
+            else *ptr = S[j * PITCH + i];
+        }
     }
 
     // counters: net deposits (one atomic per warp) and the tracked height of site (0,0)

@@ -440,9 +440,8 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     if (dom >= P.ndom) return;
 
     // ---- a1: per-MCS control from the global stream (:144, :150; R10) --------------------------
-    const bool half = DEAD && P.dev == kDevDBh;      // DB with t_async = 1/2: this launch is interval P.si (R27)
-    uint32_t Gw[4];
-    philox4x32_10(half ? P.si : 0u, 0u, kTagGlobal << 30, t, rk, Gw);
+    uint32_t Gw[4];                                  // dead-border layers: this launch is interval P.si of the sweep (R27)
+    philox4x32_10(DEAD ? P.si : 0u, 0u, kTagGlobal << 30, t, rk, Gw);
     uint32_t gx, gy, set, dead_w;
     if constexpr (!DEAD) {
         const uint32_t Ox = P.dev == kDevDTr ? (Gw[0] & Lm) : 0u, Oy = P.dev == kDevDTr ? (Gw[1] & Lm) : 0u;
@@ -455,12 +454,12 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     } else {
         uint32_t Ox = Gw[0] & Lm, Oy = Gw[1] & Lm;
         if (P.dev == kDevCDB) { Ox &= ~3u; Oy &= ~3u; }                 // :166 coarse grid
-        set = half ? P.si : 0u;
+        set = P.si;
         const uint32_t lnt = P.log2L - LOG2D;
         const uint32_t I = dom & ((1u << lnt) - 1u), J = dom >> lnt;
         gx = (Ox + (I << LOG2D)) & Lm;
         gy = (Oy + (J << LOG2D)) & Lm;
-        dead_w = P.dev == kDevCDB ? 1u : 5u;                            // :166, R22
+        dead_w = P.dead_w;                                              // :166, R22/R28
     }
     const uint32_t offx = gx & 3u, offy = gy & 3u;
     const uint32_t LW = L >> 2, LWm = LW - 1u, wx0 = gx >> 2, wy0 = gy >> 2;
@@ -473,6 +472,10 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     const uint32_t nrow = DEAD ? ((offy + (uint32_t)D - dead_w) >> 2) + 1u : (uint32_t)NW;
     auto kept = [&](uint32_t iw, uint32_t jw) -> bool { return !DEAD || (iw < ncol && jw < nrow); };
     auto word_ptr = [&](uint32_t iw, uint32_t jw) -> uint32_t* { return lat + (size_t)((wy0 + jw) & LWm) * LW + ((wx0 + iw) & LWm); };
+    auto put_word = [&](uint32_t iw, uint32_t jw, uint32_t word) {
+        if constexpr (DEAD) store_tile_word(word_ptr(iw, jw), word, iw, jw, offx, offy, (uint32_t)D, dead_w);
+        else *word_ptr(iw, jw) = word;
+    };
 
     // Programmatic dependent launch: the launches of one MCS depend on each other (kernel boundary = the device-wide
     // synchronisation of :144), but everything above touches no global memory, so the next launch's CTAs may take
@@ -586,8 +589,8 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     const bool onedir = BLK == kBlkSync || P.P16 == 0u || P.Q16 == 0u;
     const uint32_t T16 = P.Q16 == 0u ? P.P16 : P.Q16;
     const uint32_t dead_lim = (uint32_t)D - dead_w;
-    const uint32_t k4_begin = half ? P.si * (uint32_t)(SH::NSTEP / 8) : 0u;
-    const uint32_t k4_end = half ? k4_begin + (uint32_t)(SH::NSTEP / 8) : (uint32_t)(SH::NSTEP / 4);
+    const uint32_t k4_per = DEAD ? (uint32_t)(SH::NSTEP / 4) >> P.ka : (uint32_t)(SH::NSTEP / 4);   // steps of this interval
+    const uint32_t k4_begin = DEAD ? P.si * k4_per : 0u, k4_end = k4_begin + k4_per;
 #define OCT_RUN(ONEDIR, ALWAYS) \
     run_steps<SH, BLK, ONEDIR, ALWAYS, DEAD>(Sb, BT, tg, grp, wmask, c2b, c2c, t, rk, P.P16, P.Q16, P.dtr_mask, dead_lim, k4_begin, k4_end)
     if (onedir && T16 == 65536u) OCT_RUN(true, true);
@@ -603,17 +606,17 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
         for (uint32_t jw = 0; jw < (uint32_t)NW; ++jw) {
             if (!kept(iw, jw)) continue;
             const uint32_t word = gather_word<SH>(S, iw, jw);
-            *word_ptr(iw, jw) = word;
+            put_word(iw, jw, word);
             net -= x_moment(word, iw);
         }
         if (kept(NW - 1, tg)) {
             const uint32_t word = gather_word_rot<SH>(S, NW - 1, tg, tg >> 1);
-            *word_ptr(NW - 1, tg) = word;
+            put_word(NW - 1, tg, word);
             net -= x_moment(word, NW - 1);
         }
         if (tg == 0u && kept(NW - 1, NW - 1)) {
             const uint32_t word = gather_word<SH>(S, NW - 1, NW - 1);
-            *word_ptr(NW - 1, NW - 1) = word;
+            put_word(NW - 1, NW - 1, word);
             net -= x_moment(word, NW - 1);
         }
     } else if constexpr (SH::FAST_17) {
@@ -622,12 +625,12 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
         for (uint32_t jw = hi; jw < (uint32_t)NW; jw += 2) {
             if (!kept(iw, jw)) continue;
             const uint32_t word = gather_word<SH>(S, iw, jw);
-            *word_ptr(iw, jw) = word;
+            put_word(iw, jw, word);
             net -= x_moment(word, iw);
         }
         if (tg < (uint32_t)NW && kept(NW - 1, tg)) {
             const uint32_t word = gather_word_rot<SH>(S, NW - 1, tg, tg >> 1);
-            *word_ptr(NW - 1, tg) = word;
+            put_word(NW - 1, tg, word);
             net -= x_moment(word, NW - 1);
         }
     } else {
@@ -635,7 +638,7 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
             const uint32_t jw = idx / NW, iw = idx - jw * NW;
             if (!kept(iw, jw)) continue;
             const uint32_t word = gather_word<SH>(S, iw, jw);
-            *word_ptr(iw, jw) = word;
+            put_word(iw, jw, word);
             net -= x_moment(word, iw);
         }
     }

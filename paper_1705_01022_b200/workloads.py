@@ -13,20 +13,23 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-# ---- public scheme code (include/oct.h): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 -------------
+# ---- public scheme code (include/oct.h): dev | blk<<4 | tcx<<8 | tcy<<12 | log2D<<16 | ka<<21 | w<<23 ----
 DEV_DTR, DEV_DT, DEV_DB, DEV_CDB, DEV_DBH = 0, 1, 2, 3, 4
 BLK_DB, BLK_DB_DELAYED, BLK_DT, BLK_DTR = 0, 1, 2, 3
 INIT_FLAT, INIT_FLAT_SHIFTED, INIT_FROM_DEVICE = 0, 1, 2
 
 
-def scheme_code(dev: int, blk: int, log2D: int, tcx: int = 1, tcy: int = 1) -> int:
-    return dev | (blk << 4) | (tcx << 8) | (tcy << 12) | (log2D << 16)
+def scheme_code(dev: int, blk: int, log2D: int, tcx: int = 1, tcy: int = 1, ka: int = 0, w: int = 0) -> int:
+    """ka: t_async = 2^-ka MCS; w: explicit dead-border width, 0 = the scheme's own (DB / cDB only)."""
+    return dev | (blk << 4) | (tcx << 8) | (tcy << 12) | (log2D << 16) | (ka << 21) | (w << 23)
 
 
 def scheme_name(code: int) -> str:
     dev, blk = code & 15, (code >> 4) & 15
+    ka, w = (code >> 21) & 3, (code >> 23) & 7
     return (["DTr", "DT", "DB", "cDB", "DBh"][dev] + ["DB", "DBd", "DT", "DTr"][blk]
-            + f",TC={(code >> 8) & 15},{(code >> 12) & 15},D={1 << ((code >> 16) & 31)}")
+            + f",TC={(code >> 8) & 15},{(code >> 12) & 15},D={1 << ((code >> 16) & 31)}"
+            + (f",tasync=1/{1 << ka}" if ka else "") + (f",w={w}" if w else ""))
 
 
 @dataclass(frozen=True)

@@ -87,6 +87,21 @@ def test_host_helpers_are_exact_rationals_rounded_once():
     assert binding.oct_w2_from_sums(256, 256 * 256 // 2, 256 * 256 // 2) == 0.25       # flat start (R5)
 
 
+def test_t_async_and_width_fields():
+    ok = binding.oct_scheme_supported
+    import oracle
+    for dev in (wl.DEV_DTR, wl.DEV_DT, wl.DEV_DB, wl.DEV_CDB, wl.DEV_DBH):
+        for ka in (0, 1, 2, 3):
+            for w in (0, 1, 5, 7):
+                for tc in (0, 1):
+                    code = wl.scheme_code(dev, wl.BLK_DB, 6, tc, tc, ka, w)
+                    assert ok(256, code) == (oracle.lib().orc_check_scheme(256, code) == 0), (dev, ka, w, tc)
+    assert ok(256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 2, 1)) and not ok(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 1, 1, 1, 0))
+    assert not ok(256, 1 << 26)
+    assert binding.oct_time_per_sweep(256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 2, 1)) == pytest.approx((63 / 64) ** 2)
+    assert binding.oct_time_per_sweep(256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 6, 1, 1, 0, 3)) == pytest.approx((61 / 64) ** 2)
+
+
 def test_time_per_sweep_eq9():
     # Eq. (9) with reading R9: a DB sweep lasts (N - N_border)/N MCS
     assert binding.oct_time_per_sweep(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6)) == 1.0

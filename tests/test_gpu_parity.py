@@ -69,6 +69,16 @@ SMALL = [
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 6, 2, 2), 0.6, 0.4, 5),
     (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 6),          # ... of which one has no domain (4 tiles, odd split)
     (64, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 5), 0.5, 0.5, 10),               # D = 32 TC=1,1: half-warp groups, one tile
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 2, 0), 1.0, 0.0, 8),    # t_async = 1/4 MCS
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 0, 1), 1.0, 0.0, 10),   # border width 1 with a FREE origin: shared words
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 1, 1), 0.7, 0.3, 8),
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DT, 6, 1, 1, 2, 3), 0.6, 0.4, 6),
+    (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 5, 1, 1, 2, 2), 0.9, 0.1, 8),
+    (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 6, 1, 1, 2, 3), 1.0, 0.0, 6),
+    (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 7, 1, 1, 1, 1), 1.0, 0.0, 4),
+    (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8, 1, 1, 2, 1), 0.8, 0.2, 3),    # bit-packed kernel only (D = 256)
+    (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 2, 2, 1, 1), 1.0, 0.0, 6),    # two domains per warp
+    (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 2, 1), 0.7, 0.3, 10),    # L = D, width 1: the tile is its own neighbour
     (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 5), 0.5, 0.5, 16),
     (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 0, 0), 1.0, 0.0, 8),
     (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 5, 2, 2), 0.8, 0.2, 8),
