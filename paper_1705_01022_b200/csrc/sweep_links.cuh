@@ -5,12 +5,12 @@
 // Why a second layout (profiles/r1_a_*.md): on the bit-packed window the update test costs ~115 SASS
 // instructions per attempt, almost all of them shift/mask arithmetic and shared-memory atomics, and the
 // ALU pipe binds.  Here the window is unpacked ONCE per domain sweep into one 32-bit *entry* per site that
-// carries the four links of that site, one byte each:
+// carries the four links of that site, one byte each (0x00 = slope -1, 0xFF = slope +1):
 //      byte 0  W = sigma_x(x,y)     byte 1  E = sigma_x(x+1,y)
 //      byte 2  S = sigma_y(x,y)     byte 3  N = sigma_y(x,y+1)                      (:140, R3)
 // so that
 //   * the eligibility test of Eq. (1) (:27-34) is one LDS.32 and one compare: local minimum
-//     (W,E,S,N) = (0,1,0,1) <=> entry == 0x01000100, local maximum <=> entry == 0x00010001;
+//     (W,E,S,N) = (0,1,0,1) <=> entry == 0xFF00FF00, local maximum <=> entry == 0x00FF00FF;
 //   * an accepted update is five plain stores: the site's own entry and one byte in each of the four
 //     neighbouring entries (every link is stored twice, once per end site).  No atomics are needed:
 //     a link can only be changed by an update at one of its two end sites, two nearest-neighbour sites
@@ -19,7 +19,10 @@
 //     stray byte writes in their E/N bytes only, which are never read and never written back.
 //   * the window is kept in the lattice's own 4-site word alignment (pitch D+4 entries), so stage-in
 //     expands a packed word into four 128-bit stores and stage-out gathers it back from four 128-bit
-//     loads with multiply-shift bit gathers.
+//     loads.  Both are byte permutes (profiles/r2_sweep.md: the kernel is bound by the instruction issue
+//     rate at three warps per scheduler, and staging was 39 % of its instructions): a link byte is the
+//     SIGN-REPLICATED top bit of a byte of a shifted copy of the packed word (PRMT with selector bit 3),
+//     12 shifts + 24 permutes per 16 entries; the way back is 2 permutes, 2 masks and one multiply per row.
 // Everything else (Philox streams, per-MCS control, cell geometry, phases) is as in sweep.cuh and
 // follows the same readings R10-R19 of DESIGN.md.
 #pragma once
@@ -32,8 +35,8 @@
 
 namespace octb {
 
-constexpr uint32_t kEntryMin = 0x01000100u;   // (W,E,S,N) = (0,1,0,1): local minimum, Eq. (1)
-constexpr uint32_t kEntryMax = 0x00010001u;   // (1,0,1,0): local maximum
+constexpr uint32_t kEntryMin = 0xFF00FF00u;   // (W,E,S,N) = (0,1,0,1): local minimum, Eq. (1); a set link is the byte 0xFF
+constexpr uint32_t kEntryMax = 0x00FF00FFu;   // (1,0,1,0): local maximum
 
 // G_ = threads of the worker group that owns one domain: a multiple of 32 (one or several warps), or 16 -- two
 // domains per warp, for domains with only 16 thread cells (TC=2,2 at D = 64: the paper's second production
@@ -68,37 +71,44 @@ struct LinkShape {
     static_assert(CX <= D && CY <= D, "cell larger than domain");
 };
 
-// bits 0,2,4,6 of b -> bit 0 of bytes 0,1,2,3 (multiply-shift scatter; partial products never collide
-// in a way that carries into a kept bit)
-__device__ __forceinline__ uint32_t scatter4(uint32_t b) { return ((b & 0x55u) * 0x41041u) & 0x01010101u; }
-
-// four entries of one site row from the scattered slope bytes: sx / sy = sigma_x / sigma_y of the four sites,
-// sxe = sigma_x of their east neighbours, syn = sigma_y of their north neighbours (4 x 4 byte transpose by PRMT)
-__device__ __forceinline__ uint4 entries_of_row(uint32_t sx, uint32_t sxe, uint32_t sy, uint32_t syn)
+// byte permute with the full 4-bit selectors of PTX prmt: selector nibble n picks byte (n & 7) of {a, b}; n & 8 replicates
+// that byte's top bit over the whole result byte (0x00 / 0xFF)
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel)
 {
-    const uint32_t t0 = __byte_perm(sx, sxe, 0x5140), t1 = __byte_perm(sx, sxe, 0x7362);
-    const uint32_t u0 = __byte_perm(sy, syn, 0x5140), u1 = __byte_perm(sy, syn, 0x7362);
-    uint4 q;
-    q.x = __byte_perm(t0, u0, 0x5410); q.y = __byte_perm(t0, u0, 0x7632);
-    q.z = __byte_perm(t1, u1, 0x5410); q.w = __byte_perm(t1, u1, 0x7632);
-    return q;
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
 }
 
 // Expand packed word A (with its east neighbour Ew and north neighbour Nw) into 16 entries.
+// Shifted copies of A put one link bit of every site row at the top of that row's byte: sigma_x of site i at the top
+// of the bytes of A << (7 - 2i), sigma_y of site i at the top of the bytes of A << (6 - 2i); sign-replicating permutes
+// then write the link bytes straight into place: (W,E) pairs of two rows from one permute, then one permute per entry.
 template <class SH>
 __device__ __forceinline__ void expand_word(uint32_t* __restrict__ S, uint32_t iw, uint32_t jw, uint32_t A,
                                             uint32_t Ew, uint32_t Nw)
 {
-    uint32_t sy[5];
+    uint32_t BW[5], BS[4], BN[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) sy[j] = scatter4(A >> (8 * j + 1));
-    sy[4] = scatter4(Nw >> 1);
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const uint32_t sx = scatter4(A >> (8 * j));
-        const uint32_t sxe = (sx >> 8) | (((Ew >> (8 * j)) & 1u) << 24);   // sigma_x of the site to the east
-        *reinterpret_cast<uint4*>(S + (4 * jw + j) * SH::P + 4 * iw) = entries_of_row(sx, sxe, sy[j], sy[j + 1]);
+    for (int i = 0; i < 4; ++i) {
+        BW[i] = A << (7 - 2 * i);                                 // byte j, top bit: sigma_x(site i, row j)
+        BS[i] = A << (6 - 2 * i);                                 //                  sigma_y(site i, row j)
+        BN[i] = __funnelshift_r(A, Nw, 18 + 2 * i);               // byte 0: sigma_y(site i, row 3); byte 1: sigma_y(site i, row 0 of Nw)
     }
+    BW[4] = Ew << 7;                                              // sigma_x of the east word's site 0
+    uint32_t e[4][4];                                             // e[j][i]: entry of site i of row j
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t we01 = prmt(BW[i], BW[i + 1], 0xD9C8u);    // (W, E) of rows 0 and 1
+        const uint32_t we23 = prmt(BW[i], BW[i + 1], 0xFBEAu);    // (W, E) of rows 2 and 3
+        e[0][i] = prmt(we01, BS[i], 0xDC10u);                     // S = row 0, N = row 1 of sigma_y
+        e[1][i] = prmt(we01, BS[i], 0xED32u);
+        e[2][i] = prmt(we23, BS[i], 0xFE10u);
+        e[3][i] = prmt(we23, BN[i], 0xDC32u);                     // N from the north word
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+        *reinterpret_cast<uint4*>(S + (4 * jw + j) * SH::P + 4 * iw) = make_uint4(e[j][0], e[j][1], e[j][2], e[j][3]);
 }
 
 // The same with the four site rows visited in the order (j + rot) & 3.  Used for the last window column, where the
@@ -111,29 +121,37 @@ __device__ __forceinline__ void expand_word_rot(uint32_t* __restrict__ S, uint32
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const uint32_t jj = ((uint32_t)j + rot) & 3u;
-        const uint32_t lo = __funnelshift_r(A, Nw, 8u * jj);               // (Nw:A) >> 8 jj: rows jj.. of A, then row 0 of Nw
-        const uint32_t sx = scatter4(lo);
-        const uint32_t sxe = (sx >> 8) | (((Ew >> (8u * jj)) & 1u) << 24);
-        *reinterpret_cast<uint4*>(S + (4 * jw + jj) * SH::P + 4 * iw) = entries_of_row(sx, sxe, scatter4(lo >> 1), scatter4(lo >> 9));
+        const uint32_t lo = __funnelshift_r(A, Nw, 8u * jj);      // byte 0: row jj, byte 1: the row north of it
+        const uint32_t le = (Ew >> (8u * jj)) << 7;               // byte 0, top bit: sigma_x of the east word's site 0 in row jj
+        uint32_t q[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t we = prmt(lo << (7 - 2 * i), i < 3 ? lo << ((5 - 2 * i) & 31) : le, 0x00C8u);
+            q[i] = prmt(we, lo << (6 - 2 * i), 0xDC10u);
+        }
+        *reinterpret_cast<uint4*>(S + (4 * jw + jj) * SH::P + 4 * iw) = make_uint4(q[0], q[1], q[2], q[3]);
     }
 }
 
-// own links (bytes 0 and 2) of the four entries of one site row -> the row's 8 bits of the packed word
-__device__ __forceinline__ uint32_t row_bits(const uint4 q)
+// own links (bytes 0 and 2) of the four entries of one site row -> the row's 8 bits of the packed word, in the TOP byte
+// of the result: two permutes line the eight link bytes up, two masks keep one distinct bit of each, and a multiply
+// adds the four bytes (no carries: the bits are distinct)
+__device__ __forceinline__ uint32_t row_bits_top(const uint4 q)
 {
-    const uint32_t z = q.x + 4u * q.y + 16u * q.z + 64u * q.w;           // W bits at 0,2,4,6; S bits at 16,18,20,22
-    return (z & 0x55u) | ((z >> 15) & 0xAAu);
+    const uint32_t t01 = prmt(q.x, q.y, 0x6240u);                 // (W0, W1, S0, S1)
+    const uint32_t t23 = prmt(q.z, q.w, 0x6240u);                 // (W2, W3, S2, S3)
+    return ((t01 & 0x08020401u) | (t23 & 0x80204010u)) * 0x01010101u;
 }
 
 // Gather the own links of 16 entries back into one packed word.
 template <class SH>
 __device__ __forceinline__ uint32_t gather_word(const uint32_t* __restrict__ S, uint32_t iw, uint32_t jw)
 {
-    uint32_t word = 0;
+    uint32_t p[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j)
-        word |= row_bits(*reinterpret_cast<const uint4*>(S + (4 * jw + j) * SH::P + 4 * iw)) << (8 * j);
-    return word;
+        p[j] = row_bits_top(*reinterpret_cast<const uint4*>(S + (4 * jw + j) * SH::P + 4 * iw));
+    return prmt(prmt(p[0], p[1], 0x0073u), prmt(p[2], p[3], 0x0073u), 0x5410u);
 }
 
 template <class SH>
@@ -143,29 +161,19 @@ __device__ __forceinline__ uint32_t gather_word_rot(const uint32_t* __restrict__
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const uint32_t jj = ((uint32_t)j + rot) & 3u;
-        word |= row_bits(*reinterpret_cast<const uint4*>(S + (4 * jw + jj) * SH::P + 4 * iw)) << (8u * jj);
+        word |= (row_bits_top(*reinterpret_cast<const uint4*>(S + (4 * jw + jj) * SH::P + 4 * iw)) >> 24) << (8u * jj);
     }
     return word;
 }
 
-// entry index y*P + x of the site packed as v = x | y << 8 (fields may hold x + D, y + D: cells wrap inside
-// the domain, R14): mask both fields at once, then y*P + x = vm + y*(P - 256)
+// entry index soff + y*P + x of the site packed as v = x | y << 8 (fields may hold x + D, y + D: cells wrap inside
+// the domain, R14): mask both fields at once, then one byte dot product (x, y, 0, 0) . (1, P, 0, 0) + soff
 template <class SH>
-__device__ __forceinline__ uint32_t site_index(uint32_t v)
+__device__ __forceinline__ uint32_t site_index(uint32_t v, uint32_t soff)
 {
+    static_assert(SH::P <= 255, "the pitch is a byte weight of the dot product");
     const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
-    return (vm >> 8) * (uint32_t)(SH::P - 256) + vm;
-}
-
-// First moment sum_x x * b(x) of the sigma_x bits of packed window word (iw, .), x = 4*iw + i.  The sweep
-// does not count its accepted updates: inside a window row the heights of the sites west and east of the
-// active span are fixed during the launch, so sum_x delta b(x) = 0 and the rise of the surface is
-// sum_sites delta h = -2 sum x * delta b(x); every deposit raises one site by 2, hence
-//     deposits - removals = sum over window words of (moment before - moment after).
-__device__ __forceinline__ int x_moment(uint32_t word, uint32_t iw)
-{
-    const uint32_t m = word & 0x55555555u;
-    return (int)(4u * iw * __popc(m) + __popc(m & 0x44444444u) + 2u * __popc(m & 0x50505050u));
+    return __dp4a(vm, (uint32_t)(1 | (SH::P << 8)), soff);
 }
 
 // Carry out an accepted update at entry index `i` (relative to Sb): the site's four links flip.
@@ -174,7 +182,7 @@ template <class SH>
 __device__ __forceinline__ void flip_links(uint32_t* Sb, uint32_t i, bool up)
 {
     unsigned char* B = reinterpret_cast<unsigned char*>(Sb + i);
-    const unsigned char v1 = up ? 1 : 0, v0 = up ? 0 : 1;
+    const unsigned char v1 = up ? 0xFF : 0, v0 = up ? 0 : 0xFF;
     Sb[i] = up ? kEntryMax : kEntryMin;
     B[-4 + 1] = v1;                 // west neighbour's E link  = sigma_x(x,y)
     B[+4 + 0] = v0;                 // east neighbour's W link  = sigma_x(x+1,y)
@@ -203,11 +211,12 @@ struct Rule {
             return (e == kEntryMin && r16 < P16) ? 1 : ((e == kEntryMax && r16 < Q16) ? -1 : 0);
         }
     }
+    // carry out decision d at entry i and count it in net (deposits - removals; ONEDIR counts updates, the caller signs them)
     template <class SH>
-    __device__ __forceinline__ void apply(uint32_t* Sb, uint32_t i, int d) const
+    __device__ __forceinline__ void apply(uint32_t* Sb, uint32_t i, int d, int& net) const
     {
-        if constexpr (ONEDIR) { if (d != 0) flip_links<SH>(Sb, i, dep); }
-        else { if (d != 0) flip_links<SH>(Sb, i, d > 0); }
+        if constexpr (ONEDIR) { if (d != 0) { flip_links<SH>(Sb, i, dep); ++net; } }
+        else { if (d != 0) { flip_links<SH>(Sb, i, d > 0); net += d; } }
     }
 };
 
@@ -225,63 +234,14 @@ __device__ __forceinline__ void links_sync(int grp, uint32_t wmask)
     }
 }
 
-#ifndef OCT_LINKS_MERGE
-#define OCT_LINKS_MERGE 0     // 0: every cell slot of a lane issues its own group of five stores (round 1)
-#endif
-
-// flip_links under a predicate, as five predicated stores (no branch: the merged store group below must stay
-// straight-line code, a divergent branch per step costs more than the stores it would skip)
-template <class SH>
-__device__ __forceinline__ void flip_links_if(bool on, uint32_t* Sb, uint32_t i, bool up)
-{
-    const uint32_t a = (uint32_t)__cvta_generic_to_shared(Sb + i);
-    const uint32_t e = up ? kEntryMax : kEntryMin, v1 = up ? 1u : 0u, v0 = up ? 0u : 1u;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t"
-        "@p st.shared.u32 [%1], %2;\n\t"
-        "@p st.shared.u8 [%1+-3], %3;\n\t"          // west neighbour's E link
-        "@p st.shared.u8 [%1+4], %4;\n\t"           // east neighbour's W link
-        "@p st.shared.u8 [%1+%5], %3;\n\t"          // south neighbour's N link
-        "@p st.shared.u8 [%1+%6], %4;\n\t}"         // north neighbour's S link
-        :: "r"((uint32_t)on), "r"(a), "r"(e), "r"(v1), "r"(v0), "n"(-4 * SH::P + 3), "n"(4 * SH::P + 2) : "memory");
-}
-
-// Carry out the decisions of one collective step.  With two cells per lane the accepted updates are spread thinly
-// (about 6 of 32 lanes per cell slot, and every store instruction costs a shared-memory wavefront or more however few
-// lanes take part), so the two slots are merged into ONE group of five stores: a lane with two accepted updates hands
-// its second one to lane ^ 16 if that lane has none (one shuffle); what is left over -- both lanes busy, seldom --
-// goes in a second, warp-uniformly skipped group.  Which lane performs a store does not matter: the updates of a
-// phase touch disjoint links (R15/R16).
-template <class SH, bool ONEDIR, bool ALWAYS, int CPT>
-__device__ __forceinline__ void apply_step(const Rule<ONEDIR, ALWAYS>& rule, uint32_t* Sb, const uint32_t (&idx)[CPT], const int (&dec)[CPT],
-                                           uint32_t wmask)
-{
-    if constexpr (OCT_LINKS_MERGE && CPT == 2 && SH::G >= 32) {
-        const bool a0 = dec[0] != 0, a1 = dec[1] != 0;
-        const bool two = a0 && a1, none = !(a0 || a1);
-        uint32_t offer = idx[1] | (two ? 0x80000000u : 0u) | (none ? 0x40000000u : 0u);
-        if constexpr (!ONEDIR) offer |= dec[1] > 0 ? 0x20000000u : 0u;
-        const uint32_t got = __shfl_xor_sync(0xFFFFFFFFu, offer, 16);
-        const bool take = none && (got >> 31);                 // the partner's second update is carried out here
-        const bool given = two && ((got >> 30) & 1u);          // ... and this lane's second one over there
-        const uint32_t i1 = take ? (got & 0xFFFFu) : (a0 ? idx[0] : idx[1]);
-        bool up1 = rule.dep, up2 = rule.dep;
-        if constexpr (!ONEDIR) { up1 = take ? (got & 0x20000000u) != 0u : (a0 ? dec[0] > 0 : dec[1] > 0); up2 = dec[1] > 0; }
-        flip_links_if<SH>(a0 || a1 || take, Sb, i1, up1);
-        const bool rest = two && !given;
-        if (__any_sync(0xFFFFFFFFu, rest)) flip_links_if<SH>(rest, Sb, idx[1], up2);
-    } else {
-#pragma unroll
-        for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
-    }
-}
-
 // The collective single-hit steps of one domain sweep (:168-174).
 // DEAD: dead-border device layer (:135): attempts whose domain-local x or y is >= dead_lim are not carried out.
+// S = row 0 of the window, soff = entry index of the domain's site (0,0) in it.  Returns deposits - removals of the
+// calling lane's cells.
 template <class SH, int BLK, bool ONEDIR, bool ALWAYS, bool DEAD>
-__device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, uint32_t* __restrict__ BT, uint32_t tg, int grp, uint32_t wmask,
-                                         uint32_t c2b, uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16, uint32_t dtr_mask,
-                                         uint32_t dead_lim, uint32_t k4_begin, uint32_t k4_end)
+__device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff, uint32_t* __restrict__ BT, uint32_t tg, int grp, uint32_t wmask,
+                                        uint32_t c2b, uint32_t c2c, uint32_t t, const PhiloxRoundKeys& rk, uint32_t P16, uint32_t Q16, uint32_t dtr_mask,
+                                        uint32_t dead_lim, uint32_t k4_begin, uint32_t k4_end)
 {
     constexpr int CX = SH::CX, CY = SH::CY, G = SH::G, CPT = SH::CPT;
     constexpr uint32_t LOG2NCX = 0 + (SH::NCX == 1 ? 0 : SH::NCX == 2 ? 1 : SH::NCX == 4 ? 2 : SH::NCX == 8 ? 3 : SH::NCX == 16 ? 4 : 5);
@@ -300,13 +260,14 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, uint32_t* _
 
     // decision for the site packed in v (x | y << 8 before wrapping); idx receives its entry index
     auto decide_site = [&](uint32_t v, uint32_t w, uint32_t& idx) -> int {
-        idx = site_index<SH>(v);
+        idx = site_index<SH>(v, soff);
         if constexpr (DEAD) {
             const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
             if ((vm & 0xFFu) >= dead_lim || (vm >> 8) >= dead_lim) return 0;      // dead border: not carried out
         }
-        return rule.decide(Sb[idx], w);
+        return rule.decide(S[idx], w);
     };
+    int net = 0;                                     // accepted updates of this lane's cells (counted under the stores' predicate)
 
     // a few groups of four steps per loop trip: the next groups' Philox rounds fill the issue slots the current
     // group's shared-memory round trips leave open (+3 % at D = 64, +8 % at D = 128 over no unrolling)
@@ -318,6 +279,16 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, uint32_t* _
     for (uint32_t q = tg; q < RB && kb + q < k4_end; q += G) {
         uint32_t o[4];
         philox4x32_10(kb + q, 0u, c2b, t, rk, o);
+        // what the steps need of a block-step word is worked out here, once per step instead of once per warp and step:
+        // DB: the cell origin (ox, oy) (R13); DT: the quadrant's offset (R17), DTr: plus the origin (:234, R26)
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+            if constexpr (BLK == kBlkDT)
+                o[kk] = ((((o[kk] >> 16) & 1u) * (CX / 2)) | ((((o[kk] >> 17) & 1u) * (CY / 2)) << 8))
+                        + (o[kk] & dtr_mask & (uint32_t)((CX - 1) | ((CY - 1) << 8)));
+            else
+                o[kk] &= FM;
+        }
         *reinterpret_cast<uint4*>(BT + 4 * q) = make_uint4(o[0], o[1], o[2], o[3]);
     }
     links_sync<G, SH::DPB>(grp, wmask);
@@ -337,7 +308,7 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, uint32_t* _
             if constexpr (BLK == kBlkSync) {
                 // "ignoring borders" (:174) made order-free (R16): all cells decide on the state at the start
                 // of the step, then all accepted updates are carried out
-                const uint32_t sc = Bw & FM;
+                const uint32_t sc = Bw;
                 int dec[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
@@ -345,11 +316,12 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, uint32_t* _
                     dec[j] = decide_site((w & FM) + cellc[j] + sc, w, idx[j]);
                 }
                 links_sync<G, SH::DPB>(grp, wmask);
-                apply_step<SH>(rule, Sb, idx, dec, wmask);
+#pragma unroll
+                for (int j = 0; j < CPT; ++j) rule.template apply<SH>(S, idx[j], dec[j], net);
                 links_sync<G, SH::DPB>(grp, wmask);
             } else if constexpr (BLK == kBlkDelayed) {
                 // delayed borders (:174): bulk, then edges, then corners (R15)
-                const uint32_t sc = Bw & FM;
+                const uint32_t sc = Bw;
                 uint32_t cls[CPT], vv[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
@@ -362,28 +334,29 @@ __device__ __forceinline__ void run_steps(uint32_t* __restrict__ Sb, uint32_t* _
                     int dec[CPT];                    // cells of one phase never touch common links (R15): loads first
 #pragma unroll
                     for (int j = 0; j < CPT; ++j) dec[j] = cls[j] == phase ? decide_site(vv[j], rw[j][kk], idx[j]) : 0;
-#pragma unroll
-                    for (int j = 0; j < CPT; ++j) rule.template apply<SH>(Sb, idx[j], dec[j]);
+    #pragma unroll
+                    for (int j = 0; j < CPT; ++j) rule.template apply<SH>(S, idx[j], dec[j], net);
                     links_sync<G, SH::DPB>(grp, wmask);
                 }
             } else {
                 // block-layer DT (:170): one random quadrant of every cell per step (R17).  The cells of a step
                 // cannot interact, so all loads go first and the stores follow (no load waits behind a store)
                 // (block-layer DTr, :234 / R26: plus the per-step origin of block-layer DB; site_index wraps, R14)
-                const uint32_t qc = ((((Bw >> 16) & 1u) * (CX / 2)) | ((((Bw >> 17) & 1u) * (CY / 2)) << 8))
-                                    + (Bw & dtr_mask & (uint32_t)((CX - 1) | ((CY - 1) << 8)));
+                const uint32_t qc = Bw;
                 int dec[CPT];
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
                     dec[j] = decide_site((w & FM) + cellc[j] + qc, w, idx[j]);
                 }
-                apply_step<SH>(rule, Sb, idx, dec, wmask);
+#pragma unroll
+                for (int j = 0; j < CPT; ++j) rule.template apply<SH>(S, idx[j], dec[j], net);
                 links_sync<G, SH::DPB>(grp, wmask);
             }
         }
     }
     }
+    return ONEDIR && !rule.dep ? -net : net;
 }
 
 // number of set W links of the sites (0..n00-1, y00) of the domain: with n00 = x00 + 1 it is h(x00,y00) minus the
@@ -485,7 +458,6 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     asm volatile("griddepcontrol.wait;" ::: "memory");
 
     // ---- a2: stage-in (:164): packed words -> link entries -------------------------------------
-    int net = 0;                                     // deposits - removals, from the x-moments (see x_moment)
     if constexpr (SH::FAST_17 && G == 16) {
         // Half a warp, window of 17 x 17 words: lane iw holds column iw of all 17 word rows (and lane jw word (16, jw)
         // of the last column; lane 0 also (16, 16)).  Every word is loaded ONCE, all loads in flight together: the east
@@ -502,15 +474,12 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
             const uint32_t e1 = __shfl_down_sync(wmask, A[jw], 1, 16);
             const uint32_t e2 = jw < 16 ? __shfl_sync(wmask, C, jw, 16) : __shfl_sync(wmask, C16, 0, 16);
             expand_word<SH>(S, iw, jw, A[jw], iw == 15u ? e2 : e1, A[jw + 1]);
-            if (kept(iw, jw)) net += x_moment(A[jw], iw);
         }
         // last column: lane jw expands word (16, jw), lane 0 then (16, 16); its north word is the next lane's
         const uint32_t Cn = __shfl_down_sync(wmask, C, 1, 16), Cn15 = __shfl_sync(wmask, C16, 0, 16);
         expand_word_rot<SH>(S, NW - 1, tg, C, 0u, tg == 15u ? Cn15 : Cn, tg >> 1);
-        if (kept(NW - 1, tg)) net += x_moment(C, NW - 1);
         if (tg == 0u) {
             expand_word<SH>(S, NW - 1, NW - 1, C16, 0u, 0u);
-            if (kept(NW - 1, NW - 1)) net += x_moment(C16, NW - 1);
         }
     } else if constexpr (SH::FAST_17) {
         // One warp, window of 17 x 17 words.  Lanes 0-15 take the 16 leading words of an even word row, lanes 16-31 of
@@ -534,13 +503,11 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
             const uint32_t Nw = __shfl_xor_sync(0xFFFFFFFFu, hi ? A[it] : A[it + 1], 16);
             if (jw < (uint32_t)NW) {
                 expand_word<SH>(S, iw, jw, A[it], iw == 15u ? e2 : e1, Nw);
-                if (kept(iw, jw)) net += x_moment(A[it], iw);
             }
         }
         const uint32_t Cn = __shfl_down_sync(0xFFFFFFFFu, C, 1);
         if (tg < (uint32_t)NW) {
             expand_word_rot<SH>(S, NW - 1, tg, C, 0u, Cn, tg >> 1);       // the east links of this column are never read
-            if (kept(NW - 1, tg)) net += x_moment(C, NW - 1);
         }
     } else {
         constexpr int NIT = (NW * NW + G - 1) / G;   // words per thread; loaded in chunks, all loads of a chunk before its first use
@@ -569,7 +536,6 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
                 if (idx < (uint32_t)(NW * NW)) {
                     const uint32_t jw = idx / NW, iw = idx - jw * NW;
                     expand_word<SH>(S, iw, jw, A[it], Ew[it], Nw[it]);
-                    if (kept(iw, jw)) net += x_moment(A[it], iw);
                 }
             }
         }
@@ -591,11 +557,13 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     const uint32_t dead_lim = (uint32_t)D - dead_w;
     const uint32_t k4_per = DEAD ? (uint32_t)(SH::NSTEP / 4) >> P.ka : (uint32_t)(SH::NSTEP / 4);   // steps of this interval
     const uint32_t k4_begin = DEAD ? P.si * k4_per : 0u, k4_end = k4_begin + k4_per;
+    const uint32_t soff = offy * SH::P + offx;      // entry index of the domain's site (0,0)
+    int net = 0;                                     // deposits - removals of this lane's cells
 #define OCT_RUN(ONEDIR, ALWAYS) \
-    run_steps<SH, BLK, ONEDIR, ALWAYS, DEAD>(Sb, BT, tg, grp, wmask, c2b, c2c, t, rk, P.P16, P.Q16, P.dtr_mask, dead_lim, k4_begin, k4_end)
-    if (onedir && T16 == 65536u) OCT_RUN(true, true);
-    else if (onedir)             OCT_RUN(true, false);
-    else if constexpr (BLK != kBlkSync) OCT_RUN(false, false);
+    run_steps<SH, BLK, ONEDIR, ALWAYS, DEAD>(S, soff, BT, tg, grp, wmask, c2b, c2c, t, rk, P.P16, P.Q16, P.dtr_mask, dead_lim, k4_begin, k4_end)
+    if (onedir && T16 == 65536u) net = OCT_RUN(true, true);
+    else if (onedir)             net = OCT_RUN(true, false);
+    else if constexpr (BLK != kBlkSync) net = OCT_RUN(false, false);
 #undef OCT_RUN
     // every variant of run_steps ends with a group barrier: the entries are final here
 
@@ -607,17 +575,14 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
             if (!kept(iw, jw)) continue;
             const uint32_t word = gather_word<SH>(S, iw, jw);
             put_word(iw, jw, word);
-            net -= x_moment(word, iw);
         }
         if (kept(NW - 1, tg)) {
             const uint32_t word = gather_word_rot<SH>(S, NW - 1, tg, tg >> 1);
             put_word(NW - 1, tg, word);
-            net -= x_moment(word, NW - 1);
         }
         if (tg == 0u && kept(NW - 1, NW - 1)) {
             const uint32_t word = gather_word<SH>(S, NW - 1, NW - 1);
             put_word(NW - 1, NW - 1, word);
-            net -= x_moment(word, NW - 1);
         }
     } else if constexpr (SH::FAST_17) {
         const uint32_t hi = tg >> 4, iw = tg & 15u;
@@ -626,12 +591,10 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
             if (!kept(iw, jw)) continue;
             const uint32_t word = gather_word<SH>(S, iw, jw);
             put_word(iw, jw, word);
-            net -= x_moment(word, iw);
         }
         if (tg < (uint32_t)NW && kept(NW - 1, tg)) {
             const uint32_t word = gather_word_rot<SH>(S, NW - 1, tg, tg >> 1);
             put_word(NW - 1, tg, word);
-            net -= x_moment(word, NW - 1);
         }
     } else {
         for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
@@ -639,11 +602,10 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
             if (!kept(iw, jw)) continue;
             const uint32_t word = gather_word<SH>(S, iw, jw);
             put_word(iw, jw, word);
-            net -= x_moment(word, iw);
         }
     }
 
-    // counters: net deposits (one atomic per warp) and the tracked height of site (0,0): the site west
+    // counters: net deposits (counted by run_steps, one atomic per warp) and the tracked height of site (0,0): the site west
     // of the row start is inactive in this launch, so the change of h(0,0) is twice the change of the
     // number of up-links between them
     d00 += row_links_up<SH>(Sb, n00, r00, tg);
