@@ -38,43 +38,60 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+# what each translation unit includes: a unit is recompiled when one of these (or this file) is newer than its object
+UNIT_DEPS = {"oct_api.cu": ["oct_api.cu", "observe.cuh", "observe_rows.cuh", "philox.cuh", "launch.h", "sweep.cuh",
+                            os.path.join("..", "..", "include", "oct.h")],
+             "sweep_inst.cu": ["sweep_inst.cu", "launch.h", "sweep.cuh", "sweep_links.cuh", "philox.cuh"]}
+
+
+def _unit_stale(obj: str, src: str, force: bool) -> bool:
+    if force or not os.path.exists(obj):
+        return True
+    t = os.path.getmtime(obj)
+    deps = [os.path.join(CSRC, f) for f in UNIT_DEPS[src]] + [os.path.abspath(__file__)]
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
 def build(force: bool = False, verbose: bool = False, ptxas_info: str | None = None, extra_flags=()) -> str:
-    """Compile every unit (in parallel), link liboct_b200.so.  ptxas_info: optional path that receives ptxas'
-    per-kernel register / spill / shared-memory report; extra_flags: additional nvcc flags (e.g. -D switches)."""
+    """Compile the stale units (in parallel; all of them with force=True or extra_flags), link liboct_b200.so.  Objects are
+    kept under build/ (git-ignored) so that a change to one header recompiles only the units that include it.
+    ptxas_info: optional path that receives ptxas' per-kernel register / spill / shared-memory report of the units that
+    were compiled; extra_flags: additional nvcc flags (e.g. -D switches)."""
     if not (force or stale()):
         return LIB
     os.makedirs(OBJDIR, exist_ok=True)
     tag = f".tmp{os.getpid()}"
-    procs = []
+    procs, objs = [], []
     for name, src, defs in UNITS:
-        obj = os.path.join(OBJDIR, name + tag + ".o")
-        cmd = [nvcc(), *NVCC_FLAGS, *defs, *extra_flags, "-c", "-o", obj, os.path.join(CSRC, src)]
-        procs.append((name, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
-    report, failed, objs = [], None, []
+        obj = os.path.join(OBJDIR, name + ".o")
+        objs.append(obj)
+        if _unit_stale(obj, src, force or bool(extra_flags)):
+            cmd = [nvcc(), *NVCC_FLAGS, *defs, *extra_flags, "-c", "-o", obj + tag, os.path.join(CSRC, src)]
+            procs.append((name, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
+    report, failed = [], None
     for name, obj, pr in procs:
         out, err = pr.communicate()
         report.append(err)
-        objs.append(obj)
         if verbose or pr.returncode:
             print(out)
             print(err)
-        if pr.returncode and failed is None:
-            failed = f"nvcc failed on {name}:\n" + err[-4000:]
-    try:
-        if failed:
-            raise RuntimeError(failed)
-        tmp = LIB + tag
-        res = subprocess.run([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs], capture_output=True, text=True)
-        if res.returncode:
-            raise RuntimeError("link failed:\n" + res.stderr[-4000:])
-        if ptxas_info:
-            with open(ptxas_info, "w") as f:
-                f.write("".join(l for e in report for l in e.splitlines(True) if "Compile time" not in l))
-        os.replace(tmp, LIB)
-    finally:
-        for o in objs:
-            if os.path.exists(o):
-                os.unlink(o)
+        if pr.returncode:
+            if failed is None:
+                failed = f"nvcc failed on {name}:\n" + err[-4000:]
+            if os.path.exists(obj + tag):
+                os.unlink(obj + tag)
+        else:
+            os.replace(obj + tag, obj)
+    if failed:
+        raise RuntimeError(failed)
+    tmp = LIB + tag
+    res = subprocess.run([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs], capture_output=True, text=True)
+    if res.returncode:
+        raise RuntimeError("link failed:\n" + res.stderr[-4000:])
+    if ptxas_info:
+        with open(ptxas_info, "w") as f:
+            f.write("".join(l for e in report for l in e.splitlines(True) if "Compile time" not in l))
+    os.replace(tmp, LIB)
     return LIB
 
 

@@ -90,24 +90,17 @@ constexpr int kRows2Warps = 8;
 // what one pass computes (oct_observe): any combination
 enum : int { kObsW2 = 1, kObsCh = 2, kObsCs = 4 };
 
-// the four sigma_x bits of every site row of a word, one per byte lane: b[i] byte j = sigma_x(site i of row j)
-__device__ __forceinline__ void slope_bytes(uint32_t w, uint32_t (&b)[4])
-{
-    b[0] = w & kOnes; b[1] = (w >> 2) & kOnes; b[2] = (w >> 4) & kOnes; b[3] = (w >> 6) & kOnes;
-}
-
 // heights of the four sites of a word, byte-parallel over its four site rows, from the heights just west of it:
-// H_i = H_{i-1} + 2 b_i - 1 (bytes stay within [1, 255]: no borrow between byte lanes).  The subtraction issues on
-// the ALU pipe, the multiply-add on the FMA pipe; the last H is the west height of the next word.
+// H_i = H_{i-1} + 2 b_i - 1 per byte (bytes stay within [1, 255]: no carry or borrow between byte lanes, so the
+// three-input 32-bit add is four byte adds).  2 b_i is the word's bit 2i of every byte moved to bit 1.
 __device__ __forceinline__ void walk_word(uint32_t w, uint32_t& west, uint32_t (&H)[4])
 {
-    uint32_t b[4];
-    slope_bytes(w, b);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        H[i] = b[i] * 2u + (west - kOnes);
-        west = H[i];
-    }
+    constexpr uint32_t kTwos = 0x02020202u;
+    H[0] = west + ((w << 1) & kTwos) - kOnes;
+    H[1] = H[0] + ((w >> 1) & kTwos) - kOnes;
+    H[2] = H[1] + ((w >> 3) & kTwos) - kOnes;
+    H[3] = H[2] + ((w >> 5) & kTwos) - kOnes;
+    west = H[3];
 }
 
 // One pass over the packed lattice (and the snapshot) for any combination of
@@ -165,17 +158,23 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows3_kernel(const RowsParam
                 // run's sums are plain DP4A accumulations; the bias comes off once per run
                 uint32_t ba = run_start_dq(wa[0]) + 112u * kOnes, bb = 0;      // bytes left_j - s + 128
                 if constexpr (CH) bb = run_start_dq(wb[0]) + 112u * kOnes;
-                unsigned int a1 = 0, b1 = 0, qa = 0, qab = 0;                  // sum H_A, sum H_B, sum H_A^2, sum H_A H_B
+                // neighbouring columns differ by one, so H_0^2 + H_1^2 = 2 H_0 H_1 + 1 in every byte: two dot products per word
+                // give sum H^2.  (The same trick for sum H -- columns 1 and 3 plus a population count -- and the shifts as
+                // high halves of products were measured and are slower: the ALU pipe is the one that is full, profiles/r2_observables.md)
+                unsigned int a1 = 0, b1 = 0, qa = 0, qab = 0;                  // sum H_A, sum H_B, sum H_A0 H_A1 + H_A2 H_A3, sum H_A H_B
 #pragma unroll
                 for (int k = 0; k < RUN; ++k) {
                     uint32_t HA[4], HB[4];
                     walk_word(wa[k], ba, HA);
-                    if constexpr (CH) walk_word(wb[k], bb, HB);
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        a1 = __dp4a(HA[i], kOnes, a1);
-                        if constexpr (W2) qa = __dp4a(HA[i], HA[i], qa);
-                        if constexpr (CH) { b1 = __dp4a(HB[i], kOnes, b1); qab = __dp4a(HA[i], HB[i], qab); }
+                    for (int i = 0; i < 4; ++i) a1 = __dp4a(HA[i], kOnes, a1);
+                    if constexpr (W2) { qa = __dp4a(HA[0], HA[1], qa); qa = __dp4a(HA[2], HA[3], qa); }
+                    if constexpr (CH) {
+                        walk_word(wb[k], bb, HB);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) b1 = __dp4a(HB[i], kOnes, b1);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) qab = __dp4a(HA[i], HB[i], qab);
                     }
                 }
                 constexpr int nn = 16 * RUN;
@@ -183,23 +182,26 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows3_kernel(const RowsParam
                 const int ra1 = (int)a1 - 128 * nn;                                   // sum (e_A - s_A)
                 const int rb1 = (int)b1 - 128 * nn;
                 const int totA = (int)(ba & 0xFFu) - 128, totB = (int)(bb & 0xFFu) - 128;   // net slope of site row 0 over the run
-                // place the runs: exclusive scan of the runs' net slope of site row 0
-                const int inclA = warp_inclusive_scan_i32(totA, lane);
-                const long long sA = carryA + inclA - totA;
-                carryA += __shfl_sync(0xFFFFFFFFu, inclA, 31);
-                if (on) s1 += n * sA + ra1;
+                // place the runs: exclusive scan of the runs' net slope of site row 0 (both lattices in one scan: |tot| <= 64 per
+                // lane, so the two running sums share a register as 16-bit halves)
+                const int incl = warp_inclusive_scan_i32(CH ? totA + totB * 65536 : totA, lane);
+                const int last = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                const int inclA = CH ? (int)(short)(incl & 0xFFFF) : incl, lastA = CH ? (int)(short)(last & 0xFFFF) : last;
+                const int sA = carryA + inclA - totA;               // height at the start of this lane's run (32-bit: heights are int32)
+                carryA += lastA;
+                if (on) s1 += (long long)sA * (int)n + ra1;
                 if constexpr (W2) {
-                    const int q = (int)(qa - 256u * a1) + 16384 * nn;                 // sum (H - 128)^2
-                    if (on) s2 += n * sA * sA + 2 * sA * ra1 + q;
+                    const int q = (int)(2u * qa + 8u * RUN - 256u * a1) + 16384 * nn; // sum H^2 = 2 sum (H_0 H_1 + H_2 H_3) + 8 per word; minus the bias: sum (H - 128)^2
+                    if (on) s2 += ((long long)sA * sA) * n + (long long)sA * (2 * ra1) + q;
                 }
                 if constexpr (CH) {
                     const int q = (int)(qab - 128u * (a1 + b1)) + 16384 * nn;         // sum (H_A - 128)(H_B - 128)
-                    const int inclB = warp_inclusive_scan_i32(totB, lane);
-                    const long long sB = carryB + inclB - totB;
-                    carryB += __shfl_sync(0xFFFFFFFFu, inclB, 31);
+                    const int inclB = (incl - inclA) >> 16, lastB = (last - lastA) >> 16;
+                    const int sB = carryB + inclB - totB;
+                    carryB += lastB;
                     if (on) {
-                        ss += n * sB + rb1;
-                        sts += n * sA * sB + sA * rb1 + sB * ra1 + q;
+                        ss += (long long)sB * (int)n + rb1;
+                        sts += ((long long)sA * sB) * n + (long long)sA * rb1 + (long long)sB * ra1 + q;
                     }
                 }
             }

@@ -98,9 +98,22 @@ def ensemble_mean(runs, keys=("w2", "mean_h", "c_h", "c_s"), snap_t=None):
     return out
 
 
-def simulate(L, mcs, snap, p, q, code, seeds, per_decade=8, device="cuda:0", progress=None):
-    """Growth / aging run of one lattice per seed (all members in the same launches).  Returns (runs, wall seconds):
-    runs[i] = rows of seed i on the common grid, each {sweeps, t, w2, mean_h, net[, c_h, c_s]}."""
+def member_groups(n_members: int, L: int, n_groups: int = 0):
+    """Split an ensemble into groups that run on their own CUDA streams.  The launches of one group follow each other (the
+    kernel boundary is the device-wide synchronisation of PAPER.md:144), and a launch of a few thousand domains leaves the
+    GPU partly idle while its last domains finish; a second, independent group fills that tail.  0 = choose: two groups
+    for lattices small enough that one launch of all members lasts only a few waves of domains, one otherwise."""
+    if n_groups <= 0:
+        n_groups = 2 if (n_members >= 2 and L <= 8192) else 1
+    n_groups = max(1, min(n_groups, n_members))
+    size = -(-n_members // n_groups)
+    return [list(range(i, min(i + size, n_members))) for i in range(0, n_members, size)]
+
+
+def simulate(L, mcs, snap, p, q, code, seeds, per_decade=8, device="cuda:0", progress=None, n_groups=0):
+    """Growth / aging run of one lattice per seed (the members of a group in the same launches, groups on concurrent
+    streams).  Returns (runs, wall seconds): runs[i] = rows of seed i on the common grid, each
+    {sweeps, t, w2, mean_h, net[, c_h, c_s]}."""
     import torch
     N = L * L
     dt = binding.oct_time_per_sweep(L, code)                     # Eq. (9): physical MCS per sweep (1 for DT / DTr)
@@ -111,23 +124,28 @@ def simulate(L, mcs, snap, p, q, code, seeds, per_decade=8, device="cuda:0", pro
     outs = [torch.empty(16, dtype=torch.int64, device=sims[0].device) for _ in sims]
     snaps = [None] * len(sims)
     rows = [[] for _ in sims]
+    groups = member_groups(len(sims), L, n_groups)
+    streams = [torch.cuda.current_stream(sims[0].device)] if len(groups) == 1 else [torch.cuda.Stream(sims[0].device) for _ in groups]
     torch.cuda.synchronize()
     wall0 = time.perf_counter()
     t_now = 0
     for t in grid:
-        if len(sims) == 1:
-            sims[0].oct_sweep(t - t_now, p, q, code)
-        else:
-            binding.oct_sweep_batch(sims, t - t_now, p, q, code)
-        t_now = t
-        for i, sim in enumerate(sims):
-            if snap and t == snap:
-                snaps[i] = sim.oct_snapshot()
-            if snaps[i] is not None:
-                sim.oct_observe(binding.OCT_OBS_W2 | binding.OCT_OBS_CH | binding.OCT_OBS_CS, snaps[i][0], snaps[i][1], outs[i])
+        for members, stream in zip(groups, streams):
+            if len(members) == 1:
+                sims[members[0]].oct_sweep(t - t_now, p, q, code, stream=stream)
             else:
-                sim.oct_observe(binding.OCT_OBS_W2, None, None, outs[i])
-        host = torch.stack(outs).cpu().numpy()                   # one read-back per grid point (synchronises)
+                binding.oct_sweep_batch([sims[i] for i in members], t - t_now, p, q, code, stream=stream)
+        for members, stream in zip(groups, streams):
+            for i in members:
+                if snap and t == snap:
+                    snaps[i] = sims[i].oct_snapshot(stream=stream)
+                if snaps[i] is not None:
+                    sims[i].oct_observe(binding.OCT_OBS_W2 | binding.OCT_OBS_CH | binding.OCT_OBS_CS, snaps[i][0], snaps[i][1], outs[i], stream=stream)
+                else:
+                    sims[i].oct_observe(binding.OCT_OBS_W2, None, None, outs[i], stream=stream)
+        t_now = t
+        torch.cuda.synchronize()                                 # every group has delivered its sums
+        host = torch.stack(outs).cpu().numpy()                   # one read-back per grid point
         for i in range(len(sims)):
             o = [int(v) for v in host[i]]
             row = {"sweeps": t, "t": t * dt, "w2": binding.oct_w2_from_sums(L, o[0], o[1]), "mean_h": o[2] + o[0] / N, "net": o[3]}
@@ -170,13 +188,14 @@ def main(argv=None):
     ap.add_argument("--dev", type=int, default=wl.DEV_DTR)
     ap.add_argument("--blk", type=int, default=wl.BLK_DB)
     ap.add_argument("--per-decade", type=int, default=8)
+    ap.add_argument("--streams", type=int, default=0, help="ensemble: groups of members on concurrent CUDA streams (0: choose)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
 
     L, N = args.L, args.L * args.L
     code = wl.scheme_code(args.dev, args.blk, args.log2D, args.tcx, args.tcy)
     seeds = list(range(args.seed, args.seed + args.seeds))
-    runs, wall = simulate(L, args.mcs, args.snap, args.p, args.q, code, seeds, args.per_decade)
+    runs, wall = simulate(L, args.mcs, args.snap, args.p, args.q, code, seeds, args.per_decade, n_groups=args.streams)
     dt = binding.oct_time_per_sweep(L, code)
     snap_t = args.snap * dt
     for rows in runs:

@@ -48,3 +48,14 @@ def test_aging_exponent_and_its_error_use_t_over_s():
     rel = 0.1 / math.sqrt(2) * math.sqrt(2)          # each point: values 0.9x and 1.1x -> sem = 0.1 x
     assert e[1]["lambda_h_over_z_eff_err"] == pytest.approx(math.sqrt(2) * rel / math.log(2.0))
     assert run.eff_exponent_err(1.0, 0.1, 10, 0.0, 0.1, 5) is None
+
+
+def test_member_groups_partition_the_ensemble():
+    # groups are contiguous, disjoint and cover every member; one member or a large lattice stays in one group
+    for n, L, g in ((1, 1024, 0), (2, 1024, 0), (32, 1024, 0), (33, 1024, 2), (7, 1024, 4), (8, 65536, 0), (5, 1024, 9)):
+        groups = run.member_groups(n, L, g)
+        assert [i for grp in groups for i in grp] == list(range(n))
+        assert all(grp for grp in groups)
+    assert len(run.member_groups(1, 1024)) == 1 and len(run.member_groups(32, 1024)) == 2
+    assert len(run.member_groups(8, 65536)) == 1 and len(run.member_groups(5, 1024, 9)) == 5
+    assert [len(g) for g in run.member_groups(33, 1024, 2)] == [17, 16]
