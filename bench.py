@@ -37,9 +37,10 @@ N_SM, SMSP, LANES = 148, 4, 32
 # (DESIGN.md section 5.1): 1 entry load + 5 stores of an accepted update (issued whenever a lane of the warp accepts)
 # + staging 2 x (68 x 68 entries x 4 B / 128 B) per 128 warp-attempts of a 64 x 64 domain + 1/8 block-step load.
 WAVEFRONTS_MIN = 1.0 + 5.0 + 2.0 * (68 * 68 * 4 / 128.0) / 128.0 + 0.125
-# Algorithmic lane-instructions per attempt (DESIGN.md section 5.1): Philox 40/4 = 10, site select 5, entry load +
-# compare 2, five stores 5, loop/sync 1, staging per site 9.  The executed count comes from the committed ncu capture.
-I_ALG = 32.0
+# Algorithmic lane-instructions per attempt (DESIGN.md section 7): Philox 40/4 = 10, site select 5, entry load +
+# compare 2, five stores + accept count 6, loop/sync 1, staging per site 6 (permute expansion 47/16, gather 34/16, loads,
+# stores and addresses).  The executed count comes from the committed ncu capture.
+I_ALG = 30.0
 
 
 def measured_peaks():

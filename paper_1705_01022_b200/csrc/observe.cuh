@@ -2,7 +2,7 @@
 //
 // Heights are the discrete integral of the slopes (the slope field is curl-free), so
 //   h(x,y) - h(0,0) = sum_{j=1..y} sigma_y(0,j) + sum_{i=1..x} sigma_x(i,y).
-// Kernel 1 (column_anchor_kernel, here) scans column 0 once: anchor[y] = h(0,y) - h(0,0).
+// Kernel 1 (column_gather_kernel + column_anchor_kernel, here) scans column 0 once: anchor[y] = h(0,y) - h(0,0).
 // Kernel 2 (observe_rows.cuh) gives every warp one word-row (4 site rows, L/4 packed words) and either
 // stores the heights or accumulates the centred sums.  One pass over the packed lattice, no
 // intermediate arrays.  This header also holds the parameter block and the small utility kernels.
@@ -12,26 +12,48 @@
 
 namespace octb {
 
-// ---- kernel 1: anchor[y] = sum_{j=1..y} sigma_y(0,j), one CTA ---------------------------------------
-// sigma_y(0, 4wy+j) is bit 8j+1 of word (wx=0, wy).
+// ---- kernel 1: anchor[y] = sum_{j=1..y} sigma_y(0,j) -----------------------------------------------------
+// sigma_y(0, 4wy+j) is bit 8j+1 of word (wx=0, wy).  Column 0 is strided by one lattice row per word: L/4 separate
+// 32-byte sectors.  One SM cannot keep enough of them in flight (a single CTA doing the strided reads took 25 us at
+// L = 2^16, a tenth of the W^2 pass it precedes; profiles/r2_observables.md), so the column is first gathered into a compact
+// array by a grid of CTAs (column_gather_kernel) and then scanned by one CTA per lattice from coalesced loads.
+constexpr int kGatherThreads = 256;
+
+// col[k][w] = lat_k[w * LW] for the lattices k = blockIdx.y (one or two: current lattice and snapshot)
+__global__ void __launch_bounds__(kGatherThreads)
+column_gather_kernel(const uint32_t* __restrict__ lat0, const uint32_t* __restrict__ lat1, uint32_t L,
+                     uint32_t* __restrict__ col0, uint32_t* __restrict__ col1)
+{
+    const uint32_t LW = L >> 2;
+    const uint32_t w = blockIdx.x * kGatherThreads + threadIdx.x;
+    const uint32_t* lat = blockIdx.y ? lat1 : lat0;
+    uint32_t* col = blockIdx.y ? col1 : col0;
+    if (w < LW) col[w] = lat[(size_t)w * LW];
+}
+
 constexpr int kAnchorThreads = 1024;
 
 constexpr int kAnchorMaxPer = 32;      // L <= 2^17: at most 2^15 words in column 0 = 32 per thread
 
+// one CTA per lattice (blockIdx.x): inclusive scan of the gathered column; also clears the n_zero output words of the
+// reduction that follows
 __global__ void __launch_bounds__(kAnchorThreads)
-column_anchor_kernel(const uint32_t* __restrict__ lat, uint32_t L, int32_t* __restrict__ anchor)
+column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restrict__ col1, uint32_t L,
+                     int32_t* __restrict__ anchor0, int32_t* __restrict__ anchor1, unsigned long long* __restrict__ zero, int n_zero)
 {
     __shared__ int32_t part[kAnchorThreads];
+    // the sums of the pass that follows start from zero (this kernel precedes it in the stream: no separate memset)
+    if (blockIdx.x == 0 && (int)threadIdx.x < n_zero) zero[threadIdx.x] = 0ull;
+    const uint32_t* __restrict__ col = blockIdx.x ? col1 : col0;
+    int32_t* __restrict__ anchor = blockIdx.x ? anchor1 : anchor0;
     const uint32_t LW = L >> 2;
     const uint32_t per = (LW + kAnchorThreads - 1) / kAnchorThreads;     // words of column 0 per thread
     const uint32_t w0 = threadIdx.x * per;
-    // the column is strided by one lattice row per word (one sector each): issue all of this thread's loads at
-    // once and keep the words in registers for the second pass
     uint32_t v[kAnchorMaxPer];
 #pragma unroll
     for (int k = 0; k < kAnchorMaxPer; ++k) {
         const uint32_t w = w0 + k;
-        v[k] = ((uint32_t)k < per && w < LW) ? lat[(size_t)w * LW] : 0u;
+        v[k] = ((uint32_t)k < per && w < LW) ? col[w] : 0u;
     }
     int32_t sum = 0;
 #pragma unroll
@@ -48,7 +70,7 @@ column_anchor_kernel(const uint32_t* __restrict__ lat, uint32_t L, int32_t* __re
     }
     // running value entering this thread's first word.  The scan counts sigma_y(0,0) as well, which closes the
     // loop around the torus and is not part of the path from (0,0); remove it.
-    const int32_t s00 = (lat[0] >> 1) & 1u ? 1 : -1;
+    const int32_t s00 = (col[0] >> 1) & 1u ? 1 : -1;
     int32_t run = part[threadIdx.x] - sum - s00;
 #pragma unroll
     for (int k = 0; k < kAnchorMaxPer; ++k) {

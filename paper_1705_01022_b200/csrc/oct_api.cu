@@ -32,6 +32,8 @@ struct oct_ctx {
     unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws); }
     int32_t* anchorA() const { return reinterpret_cast<int32_t*>(ws + 256); }
     int32_t* anchorB() const { return reinterpret_cast<int32_t*>(ws + 256 + (size_t)L * 4); }
+    uint32_t* colA() const { return reinterpret_cast<uint32_t*>(ws + 256 + (size_t)L * 8); }          // column 0, gathered (L/4 words)
+    uint32_t* colB() const { return reinterpret_cast<uint32_t*>(ws + 256 + (size_t)L * 9); }
 };
 
 namespace {
@@ -157,10 +159,15 @@ void launch_rows(int what, const RowsParams& rp, uint32_t LW, cudaStream_t st)
     }
 }
 
-int launch_anchor(oct_ctx* c, const uint32_t* lat, int32_t* anchor, cudaStream_t st)
+// column anchors of the current lattice (and of a snapshot, latB != nullptr) into the handle's workspace: 2 small launches;
+// the second one also zeroes the n_zero int64 words at `zero` (the output of the reduction that follows)
+int launch_anchors(oct_ctx* c, const uint32_t* latB, cudaStream_t st, void* zero = nullptr, int n_zero = 0)
 {
-    column_anchor_kernel<<<1, kAnchorThreads, 0, st>>>(lat, c->L, anchor);
-    c->launches++;
+    const uint32_t LW = c->L >> 2, nlat = latB ? 2u : 1u;
+    column_gather_kernel<<<dim3((LW + kGatherThreads - 1) / kGatherThreads, nlat), kGatherThreads, 0, st>>>(c->lat, latB, c->L, c->colA(), c->colB());
+    column_anchor_kernel<<<nlat, kAnchorThreads, 0, st>>>(c->colA(), c->colB(), c->L, c->anchorA(), c->anchorB(),
+                                                         static_cast<unsigned long long*>(zero), n_zero);
+    c->launches += 2;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;
 }
@@ -171,7 +178,7 @@ extern "C" {
 
 size_t oct_lattice_bytes(uint32_t L) { return valid_L(L) ? (size_t)L * L / 4 : 0; }
 
-size_t oct_workspace_bytes(uint32_t L) { return valid_L(L) ? 256 + 2 * (size_t)L * sizeof(int32_t) : 0; }
+size_t oct_workspace_bytes(uint32_t L) { return valid_L(L) ? 256 + 10 * (size_t)L : 0; }   // counters; 2 x L int32 anchors; 2 x L/4 words of column 0
 
 int oct_create(oct_ctx** out, uint32_t L, uint64_t seed, int init, void* lattice_dev, void* workspace_dev, void* stream)
 {
@@ -373,7 +380,7 @@ int oct_heights(oct_ctx* c, int32_t* heights_dev, void* stream)
 {
     if (!c || !heights_dev || (reinterpret_cast<uintptr_t>(heights_dev) & 15u)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    int rc = launch_anchor(c, c->lat, c->anchorA(), st);
+    int rc = launch_anchors(c, nullptr, st);
     if (rc) return rc;
     RowsParams rp{};
     rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters(); rp.heights = heights_dev; rp.L = c->L;
@@ -388,8 +395,7 @@ int oct_width2(oct_ctx* c, int64_t* out_dev, void* stream)
 {
     if (!c || !out_dev) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 4 * sizeof(int64_t), st));
-    int rc = launch_anchor(c, c->lat, c->anchorA(), st);
+    int rc = launch_anchors(c, nullptr, st, out_dev, 4);
     if (rc) return rc;
     RowsParams rp{};
     rp.latA = c->lat; rp.anchorA = c->anchorA(); rp.countersA = c->counters();
@@ -416,10 +422,7 @@ int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_a
 {
     if (!c || !snapshot_dev || !snapshot_anchor_dev || !out_dev || (reinterpret_cast<uintptr_t>(snapshot_dev) & 15u)) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 5 * sizeof(int64_t), st));
-    int rc = launch_anchor(c, c->lat, c->anchorA(), st);
-    if (rc) return rc;
-    rc = launch_anchor(c, static_cast<const uint32_t*>(snapshot_dev), c->anchorB(), st);
+    int rc = launch_anchors(c, static_cast<const uint32_t*>(snapshot_dev), st, out_dev, 5);
     if (rc) return rc;
     RowsParams rp{};
     rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
@@ -455,11 +458,9 @@ int oct_observe(oct_ctx* c, int what, const void* snapshot_dev, const int64_t* s
     if (need_snap && (!snapshot_dev || (reinterpret_cast<uintptr_t>(snapshot_dev) & 15u))) return OCT_EINVAL;
     if ((what & OCT_OBS_CH) && !snapshot_anchor_dev) return OCT_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 16 * sizeof(int64_t), st));
     int rc = OCT_OK;
-    if (what & (OCT_OBS_W2 | OCT_OBS_CH)) rc = launch_anchor(c, c->lat, c->anchorA(), st);
-    if (rc) return rc;
-    if (what & OCT_OBS_CH) rc = launch_anchor(c, static_cast<const uint32_t*>(snapshot_dev), c->anchorB(), st);
+    if (what & (OCT_OBS_W2 | OCT_OBS_CH)) rc = launch_anchors(c, (what & OCT_OBS_CH) ? static_cast<const uint32_t*>(snapshot_dev) : nullptr, st, out_dev, 16);
+    else OCT_CUDA(c, cudaMemsetAsync(out_dev, 0, 16 * sizeof(int64_t), st));
     if (rc) return rc;
     RowsParams rp{};
     rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
