@@ -273,6 +273,7 @@ def main():
     ap.add_argument("--blk", type=int, default=0, help="block layer: 0 DB (the benched DTrDB), 2 DT (DTrDT, PAPER.md:268)")
     ap.add_argument("--kernel", type=int, default=0, help="OCT_OPT_KERNEL value: 0 auto, 1 bit-packed, 2 link-entry variant B")
     ap.add_argument("--also-L", type=int, default=1 << 17, help="second lattice size measured in the same run (0: none)")
+    ap.add_argument("--ensemble-L", type=int, default=1024, help="lattice edge of the ensemble (many lattices per launch) measurement (0: none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-heights", action="store_true", help="skip timing oct_heights (needs a 4*L*L byte buffer)")
@@ -410,6 +411,27 @@ def main():
         sim2.close()
         del snap2, sim2
 
+    # ---- ensembles of small lattices, all members in every launch (oct_sweep_batch; the paper's
+    # curves are means over n = 20 ... 4367 runs): sweeps only, same scheme ------------------------------------------
+    ensemble = None
+    if args.ensemble_L and world == 1:
+        ensemble = []
+        Le = args.ensemble_L
+        for n_mem in (1, 32, 256):
+            sims = [binding.Sim(Le, seed + 1 + i, wl.INIT_FLAT, device=f"cuda:{local_rank}") for i in range(n_mem)]
+            run = (lambda n: binding.oct_sweep_batch(sims, n, 1.0, 0.0, code)) if n_mem > 1 else (lambda n: sims[0].oct_sweep(n, 1.0, 0.0, code))
+            run(args.burn_in)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            Me = 200
+            a.record(stream); run(Me); b.record(stream); torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            ensemble.append({"L": Le, "members": n_mem, "mcs": Me, "ms": ms, "attempts_per_s": n_mem * Me * Le * Le / (ms * 1e-3),
+                             "domains_per_launch": n_mem * (Le >> (args.log2D + 1)) ** 2})
+            for sm in sims:
+                sm.close()
+            del sims
+
     # ---- the oracle timed on this box's host cores (rank 0, N = 1 only): bounded samples ------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -430,7 +452,7 @@ def main():
                 "ms_per_step": m["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16 and args.blk == 0) else None,
                 "dtype": "u32", "data": "synthetic", "config": workload_config(args), "clocks": m["clocks"], "e2e": e2e,
-                "gpu_launches": m["launches"], "roofline": roofline, "sustained": sustained, "also": also,
+                "gpu_launches": m["launches"], "roofline": roofline, "sustained": sustained, "also": also, "ensemble": ensemble,
                 "observables": observables, "cpu_baseline": cpu,
                 "vs_cpu_baseline": (value / world / cpu["value"]) if cpu else None,
                 "paper_context": "vs_baseline divides by PAPER.md:276's ~9e9 attempts/s (DTrDB, L=2^16, p=1, q=0) on Kepler GPUs: other hardware, "

@@ -110,7 +110,9 @@ int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* st
  * means over n = 20 ... 4367 runs, many at L <= 2^13): every kernel launch covers the
  * domains of all members (grid = domains x members, at most 256 members per launch), so small lattices fill the
  * GPU.  Each member keeps its own lattice, counters, seed and clock; its result is bit-identical to what
- * oct_sweep on that handle alone would give.  Shapes without a many-lattices kernel (D > 64, bit-packed kernel)
+ * oct_sweep on that handle alone would give.  The two halves of the ensemble run side by side -- one on `stream`, one on
+ * a helper stream of handle 0 that forks from `stream` and joins it again before the call returns -- so that the last
+ * domains of one half's launch overlap the other half's next launch; for the caller everything is ordered on `stream`.  Shapes without a many-lattices kernel (D > 64, bit-packed kernel)
  * run the members one after the other.  The kernel option of handle 0 applies.
  * Errors: as oct_sweep, plus EINVAL for n = 0, a null or repeated handle, or members of different L. */
 int oct_sweep_batch(oct_ctx* const* handles, uint32_t n, uint64_t n_mcs, double p, double q, int scheme, void* stream);

@@ -99,12 +99,12 @@ def ensemble_mean(runs, keys=("w2", "mean_h", "c_h", "c_s"), snap_t=None):
 
 
 def member_groups(n_members: int, L: int, n_groups: int = 0):
-    """Split an ensemble into groups that run on their own CUDA streams.  The launches of one group follow each other (the
-    kernel boundary is the device-wide synchronisation of PAPER.md:144), and a launch of a few thousand domains leaves the
-    GPU partly idle while its last domains finish; a second, independent group fills that tail.  0 = choose: two groups
-    for lattices small enough that one launch of all members lasts only a few waves of domains, one otherwise."""
+    """Split an ensemble into groups that run on their own CUDA streams (`--streams`).  0 = one group: oct_sweep_batch
+    itself runs the two halves of its members side by side (a launch of a few thousand domains leaves the GPU partly idle
+    while its last domains finish; the other half fills that tail), so more groups only help to overlap the per-member
+    observables of measurement-heavy runs."""
     if n_groups <= 0:
-        n_groups = 2 if (n_members >= 2 and L <= 8192) else 1
+        n_groups = 1
     n_groups = max(1, min(n_groups, n_members))
     size = -(-n_members // n_groups)
     return [list(range(i, min(i + size, n_members))) for i in range(0, n_members, size)]

@@ -56,6 +56,6 @@ def test_member_groups_partition_the_ensemble():
         groups = run.member_groups(n, L, g)
         assert [i for grp in groups for i in grp] == list(range(n))
         assert all(grp for grp in groups)
-    assert len(run.member_groups(1, 1024)) == 1 and len(run.member_groups(32, 1024)) == 2
+    assert len(run.member_groups(1, 1024)) == 1 and len(run.member_groups(32, 1024)) == 1 and len(run.member_groups(32, 1024, 2)) == 2
     assert len(run.member_groups(8, 65536)) == 1 and len(run.member_groups(5, 1024, 9)) == 5
     assert [len(g) for g in run.member_groups(33, 1024, 2)] == [17, 16]
