@@ -112,8 +112,9 @@ int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* st
  * GPU.  Each member keeps its own lattice, counters, seed and clock; its result is bit-identical to what
  * oct_sweep on that handle alone would give.  The two halves of the ensemble run side by side -- one on `stream`, one on
  * a helper stream of handle 0 that forks from `stream` and joins it again before the call returns -- so that the last
- * domains of one half's launch overlap the other half's next launch; for the caller everything is ordered on `stream`.  Shapes without a many-lattices kernel (D > 64, bit-packed kernel)
- * run the members one after the other.  The kernel option of handle 0 applies.
+ * domains of one half's launch overlap the other half's next launch; for the caller everything is ordered on `stream`.
+ * Shapes without a many-lattices kernel (D = 128 other than TC=1,1, the bit-packed kernel) run the members one after the
+ * other.  The kernel option of handle 0 applies.
  * Errors: as oct_sweep, plus EINVAL for n = 0, a null or repeated handle, or members of different L. */
 int oct_sweep_batch(oct_ctx* const* handles, uint32_t n, uint64_t n_mcs, double p, double q, int scheme, void* stream);
 
@@ -154,6 +155,14 @@ int oct_slope_autocorr(oct_ctx*, const void* snapshot_dev, int64_t* out_dev, voi
 enum { OCT_OBS_W2 = 1, OCT_OBS_CH = 2, OCT_OBS_CS = 4 };
 int oct_observe(oct_ctx*, int what, const void* snapshot_dev, const int64_t* snapshot_anchor_dev,
                 int64_t* out_dev, void* stream);
+
+/* oct_observe for n simulations of ONE lattice size in as many launches as for one (three per 64 members): a measurement
+ * point of an ensemble run.  snapshots_dev / snapshot_anchors_dev are HOST arrays of n device
+ * pointers (member i's oct_snapshot buffers; may be NULL when `what` needs none); out_dev holds n x 16 int64, member i's
+ * sums at out_dev + 16 i with the layout of oct_observe.  Results are identical to n oct_observe calls.
+ * Errors: as oct_observe, plus EINVAL for n = 0, a null handle or members of different L. */
+int oct_observe_batch(oct_ctx* const* handles, uint32_t n, int what, const void* const* snapshots_dev,
+                      const int64_t* const* snapshot_anchors_dev, int64_t* out_dev, void* stream);
 
 /* Copy `bytes` bytes of a device buffer (e.g. the sums above) to host memory.  SYNCHRONISES `stream`. */
 int oct_fetch(oct_ctx*, const void* src_dev, void* dst_host, size_t bytes, void* stream);

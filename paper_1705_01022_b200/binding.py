@@ -22,7 +22,7 @@ EXPORTS = (
     "oct_width2", "oct_snapshot", "oct_autocorr", "oct_export", "oct_upload", "oct_counters", "oct_mcs",
     "oct_destroy", "oct_strerror", "oct_last_error", "oct_launch_count", "oct_w2_from_sums", "oct_c_from_sums",
     "oct_time_per_sweep", "oct_scheme_supported", "oct_set_option", "oct_slope_autocorr", "oct_cs_from_sums",
-    "oct_sweep_batch", "oct_observe", "oct_fetch",
+    "oct_sweep_batch", "oct_observe", "oct_fetch", "oct_observe_batch",
 )
 OCT_OBS_W2, OCT_OBS_CH, OCT_OBS_CS = 1, 2, 4
 OCT_OPT_KERNEL = 1
@@ -70,6 +70,7 @@ def load(rebuild_if_stale: bool = True):
         "oct_set_option": (i32, [vp, i32, i32]),
         "oct_slope_autocorr": (i32, [vp, vp, vp, vp]), "oct_cs_from_sums": (dbl, [u64, i64, i64, i64]),
         "oct_observe": (i32, [vp, i32, vp, vp, vp, vp]), "oct_fetch": (i32, [vp, vp, vp, sz, vp]),
+        "oct_observe_batch": (i32, [C.POINTER(vp), u32, i32, C.POINTER(vp), C.POINTER(vp), vp, vp]),
     }
     for name in EXPORTS:
         fn = getattr(L, name)          # AttributeError if a declared symbol is not exported
@@ -127,6 +128,21 @@ def oct_sweep_batch(sims, n_mcs: int, p: float, q: float, scheme: int, stream=No
     rc = load().oct_sweep_batch(arr, len(sims), n_mcs, p, q, scheme, _stream_ptr(stream))
     if rc:
         raise OctError(rc, "oct_sweep_batch", load().oct_last_error(sims[0]._h).decode() if sims else "")
+
+
+def oct_observe_batch(sims, what: int, snapshots=None, anchors=None, out=None, stream=None):
+    """oct_observe for every simulation in `sims` (one lattice size) in three launches per 64 members; out: (n, 16) int64."""
+    sims = list(sims)
+    n = len(sims)
+    if out is None:
+        out = sims[0].torch.empty((n, 16), dtype=sims[0].torch.int64, device=sims[0].device)
+    hs = (C.c_void_p * n)(*[s._h for s in sims])
+    sp = (C.c_void_p * n)(*[t.data_ptr() for t in snapshots]) if snapshots is not None else None
+    ap = (C.c_void_p * n)(*[t.data_ptr() for t in anchors]) if anchors is not None else None
+    rc = load().oct_observe_batch(hs, n, what, sp, ap, out.data_ptr(), _stream_ptr(stream))
+    if rc:
+        raise OctError(rc, "oct_observe_batch", load().oct_last_error(sims[0]._h).decode() if sims else "")
+    return out
 
 
 class Sim:

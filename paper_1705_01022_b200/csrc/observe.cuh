@@ -35,17 +35,13 @@ constexpr int kAnchorThreads = 1024;
 
 constexpr int kAnchorMaxPer = 32;      // L <= 2^17: at most 2^15 words in column 0 = 32 per thread
 
-// one CTA per lattice (blockIdx.x): inclusive scan of the gathered column; also clears the n_zero output words of the
-// reduction that follows
-__global__ void __launch_bounds__(kAnchorThreads)
-column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restrict__ col1, uint32_t L,
-                     int32_t* __restrict__ anchor0, int32_t* __restrict__ anchor1, unsigned long long* __restrict__ zero, int n_zero)
+// inclusive scan of one gathered column by one CTA; also clears the n_zero output words of the reduction that follows
+// (this kernel precedes it in the stream: no separate memset)
+__device__ __forceinline__ void column_anchor_body(const uint32_t* __restrict__ col, uint32_t L, int32_t* __restrict__ anchor,
+                                                   unsigned long long* __restrict__ zero, int n_zero)
 {
     __shared__ int32_t part[kAnchorThreads];
-    // the sums of the pass that follows start from zero (this kernel precedes it in the stream: no separate memset)
-    if (blockIdx.x == 0 && (int)threadIdx.x < n_zero) zero[threadIdx.x] = 0ull;
-    const uint32_t* __restrict__ col = blockIdx.x ? col1 : col0;
-    int32_t* __restrict__ anchor = blockIdx.x ? anchor1 : anchor0;
+    if ((int)threadIdx.x < n_zero) zero[threadIdx.x] = 0ull;
     const uint32_t LW = L >> 2;
     const uint32_t per = (LW + kAnchorThreads - 1) / kAnchorThreads;     // words of column 0 per thread
     const uint32_t w0 = threadIdx.x * per;
@@ -87,6 +83,14 @@ column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restri
     }
 }
 
+// one CTA per lattice (blockIdx.x: 0 current lattice, 1 snapshot)
+__global__ void __launch_bounds__(kAnchorThreads)
+column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restrict__ col1, uint32_t L,
+                     int32_t* __restrict__ anchor0, int32_t* __restrict__ anchor1, unsigned long long* __restrict__ zero, int n_zero)
+{
+    column_anchor_body(blockIdx.x ? col1 : col0, L, blockIdx.x ? anchor1 : anchor0, zero, blockIdx.x ? 0 : n_zero);
+}
+
 // ---- kernel 2 -------------------------------------------------------------------------------------
 
 struct RowsParams {
@@ -100,6 +104,41 @@ struct RowsParams {
     unsigned long long* out;                // rows3_kernel: [0..3] W^2 sums, [4..8] C_h sums, [9..14] C_s sums
     uint32_t L;
 };
+
+// ---- the same for an ensemble (oct_observe_batch): one launch covers the members blockIdx.z / .y ---------------------
+constexpr int kMaxObsBatch = 64;
+struct ObsMember {
+    const uint32_t* latA;
+    const uint32_t* latB;                   // snapshot or nullptr
+    int32_t* anchorA;
+    int32_t* anchorB;
+    uint32_t* colA;
+    uint32_t* colB;
+    const unsigned long long* countersA;
+    const long long* snapB;
+    unsigned long long* out;                // 16 int64 of this member
+};
+struct ObsBatchParams {
+    uint32_t L;
+    int n_zero;
+    ObsMember m[kMaxObsBatch];
+};
+
+__global__ void __launch_bounds__(kGatherThreads) column_gather_batch_kernel(const __grid_constant__ ObsBatchParams BP)
+{
+    const ObsMember& mb = BP.m[blockIdx.z];
+    const uint32_t LW = BP.L >> 2;
+    const uint32_t w = blockIdx.x * kGatherThreads + threadIdx.x;
+    const uint32_t* lat = blockIdx.y ? mb.latB : mb.latA;
+    uint32_t* col = blockIdx.y ? mb.colB : mb.colA;
+    if (w < LW) col[w] = lat[(size_t)w * LW];
+}
+
+__global__ void __launch_bounds__(kAnchorThreads) column_anchor_batch_kernel(const __grid_constant__ ObsBatchParams BP)
+{
+    const ObsMember& mb = BP.m[blockIdx.y];
+    column_anchor_body(blockIdx.x ? mb.colB : mb.colA, BP.L, blockIdx.x ? mb.anchorB : mb.anchorA, mb.out, blockIdx.x ? 0 : BP.n_zero);
+}
 
 // ---- slope (lattice-gas) autocorrelation C_s(t,s), PAPER.md:85-88 --------------------------------------
 // n = slope bit.  out = {sum nx_t nx_s, sum ny_t ny_s, sum nx_t, sum ny_t, sum nx_s, sum ny_s}: one streaming

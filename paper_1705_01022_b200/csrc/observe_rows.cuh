@@ -110,7 +110,7 @@ __device__ __forceinline__ void walk_word(uint32_t w, uint32_t& west, uint32_t (
 // RUN words per lane per chunk: 16 for L >= 2048 (chunk = 512 words), 4 below (any L >= 16 works: lanes beyond L/16 idle).
 // out (int64): [0..3] = {S1, S2, c, net}; [4..8] = {S_t, S_s, S_ts, c_t, c_s}; [9..14] = {xx, yy, x_t, y_t, x_s, y_s}
 template <int WHAT, int RUN>
-__global__ void __launch_bounds__(kRows2Warps * 32) rows3_kernel(const RowsParams P)
+__device__ __forceinline__ void rows3_body(const RowsParams& P)
 {
     constexpr bool W2 = (WHAT & kObsW2) != 0, CH = (WHAT & kObsCh) != 0, CS = (WHAT & kObsCs) != 0;
     constexpr bool NEED_B = CH || CS;
@@ -253,6 +253,20 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows3_kernel(const RowsParam
             atomicAdd(&P.out[slot], t - tx);
         }
     }
+}
+
+template <int WHAT, int RUN>
+__global__ void __launch_bounds__(kRows2Warps * 32) rows3_kernel(const RowsParams P) { rows3_body<WHAT, RUN>(P); }
+
+// an ensemble: blockIdx.y picks the member (oct_observe_batch)
+template <int WHAT, int RUN>
+__global__ void __launch_bounds__(kRows2Warps * 32) rows3_batch_kernel(const __grid_constant__ ObsBatchParams BP)
+{
+    const ObsMember& mb = BP.m[blockIdx.y];
+    RowsParams P;
+    P.latA = mb.latA; P.latB = mb.latB; P.anchorA = mb.anchorA; P.anchorB = mb.anchorB; P.countersA = mb.countersA;
+    P.snapB = mb.snapB; P.heights = nullptr; P.out = mb.out; P.L = BP.L;
+    rows3_body<WHAT, RUN>(P);
 }
 
 // Heights (a8): the output (16 bytes per site row per word) dwarfs the input, so the lanes take

@@ -148,6 +148,28 @@ void launch_rows_what(const RowsParams& rp, uint32_t LW, cudaStream_t st)
     else            rows3_kernel<WHAT, 4><<<blocks, kRows2Warps * 32, 0, st>>>(rp);
 }
 
+template <int WHAT>
+void launch_rows_batch_what(const ObsBatchParams& bp, uint32_t nb, uint32_t LW, cudaStream_t st)
+{
+    const dim3 grid((LW + kRows2Warps - 1) / kRows2Warps, nb);
+    if (LW >= 512u) rows3_batch_kernel<WHAT, 16><<<grid, kRows2Warps * 32, 0, st>>>(bp);
+    else            rows3_batch_kernel<WHAT, 4><<<grid, kRows2Warps * 32, 0, st>>>(bp);
+}
+
+void launch_rows_batch(int what, const ObsBatchParams& bp, uint32_t nb, uint32_t LW, cudaStream_t st)
+{
+    switch (what) {
+        case 1: launch_rows_batch_what<1>(bp, nb, LW, st); break;
+        case 2: launch_rows_batch_what<2>(bp, nb, LW, st); break;
+        case 3: launch_rows_batch_what<3>(bp, nb, LW, st); break;
+        case 4: launch_rows_batch_what<4>(bp, nb, LW, st); break;
+        case 5: launch_rows_batch_what<5>(bp, nb, LW, st); break;
+        case 6: launch_rows_batch_what<6>(bp, nb, LW, st); break;
+        case 7: launch_rows_batch_what<7>(bp, nb, LW, st); break;
+        default: break;
+    }
+}
+
 void launch_rows(int what, const RowsParams& rp, uint32_t LW, cudaStream_t st)
 {
     switch (what) {
@@ -499,6 +521,48 @@ int oct_observe(oct_ctx* c, int what, const void* snapshot_dev, const int64_t* s
     launch_rows(what, rp, c->L >> 2, st);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());
+    return OCT_OK;
+}
+
+int oct_observe_batch(oct_ctx* const* cs, uint32_t n, int what, const void* const* snapshots_dev,
+                      const int64_t* const* snapshot_anchors_dev, int64_t* out_dev, void* stream)
+{
+    if (!cs || n == 0 || !out_dev || what <= 0 || what > (OCT_OBS_W2 | OCT_OBS_CH | OCT_OBS_CS)) return OCT_EINVAL;
+    const bool need_snap = (what & (OCT_OBS_CH | OCT_OBS_CS)) != 0, need_anchor = (what & (OCT_OBS_W2 | OCT_OBS_CH)) != 0;
+    if (need_snap && !snapshots_dev) return OCT_EINVAL;
+    if ((what & OCT_OBS_CH) && !snapshot_anchors_dev) return OCT_EINVAL;
+    for (uint32_t i = 0; i < n; ++i) {
+        if (!cs[i] || cs[i]->L != cs[0]->L) return OCT_EINVAL;
+        if (need_snap && (!snapshots_dev[i] || (reinterpret_cast<uintptr_t>(snapshots_dev[i]) & 15u))) return OCT_EINVAL;
+        if ((what & OCT_OBS_CH) && !snapshot_anchors_dev[i]) return OCT_EINVAL;
+    }
+    oct_ctx* c0 = cs[0];
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const uint32_t LW = c0->L >> 2;
+    if (!need_anchor) OCT_CUDA(c0, cudaMemsetAsync(out_dev, 0, (size_t)n * 16 * sizeof(int64_t), st));
+    ObsBatchParams bp{};
+    bp.L = c0->L; bp.n_zero = 16;
+    for (uint32_t m0 = 0; m0 < n; m0 += kMaxObsBatch) {
+        const uint32_t nb = n - m0 < (uint32_t)kMaxObsBatch ? n - m0 : (uint32_t)kMaxObsBatch;
+        for (uint32_t m = 0; m < nb; ++m) {
+            const oct_ctx* c = cs[m0 + m];
+            ObsMember& mb = bp.m[m];
+            mb.latA = c->lat; mb.latB = need_snap ? static_cast<const uint32_t*>(snapshots_dev[m0 + m]) : nullptr;
+            mb.anchorA = c->anchorA(); mb.anchorB = c->anchorB(); mb.colA = c->colA(); mb.colB = c->colB();
+            mb.countersA = c->counters();
+            mb.snapB = (what & OCT_OBS_CH) ? reinterpret_cast<const long long*>(snapshot_anchors_dev[m0 + m]) : nullptr;
+            mb.out = reinterpret_cast<unsigned long long*>(out_dev) + (size_t)(m0 + m) * 16;
+        }
+        if (need_anchor) {
+            const uint32_t nlat = (what & OCT_OBS_CH) ? 2u : 1u;
+            column_gather_batch_kernel<<<dim3((LW + kGatherThreads - 1) / kGatherThreads, nlat, nb), kGatherThreads, 0, st>>>(bp);
+            column_anchor_batch_kernel<<<dim3(nlat, nb), kAnchorThreads, 0, st>>>(bp);
+            c0->launches += 2;
+        }
+        launch_rows_batch(what, bp, nb, LW, st);
+        c0->launches++;
+        OCT_CUDA(c0, cudaGetLastError());
+    }
     return OCT_OK;
 }
 

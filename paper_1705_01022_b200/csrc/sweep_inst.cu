@@ -56,14 +56,15 @@ bool OCT_CAT(oct_find_packed_, OCT_INST_LOG2D)(int tx, int ty, int blk, SweepLau
 // Variant A is the default (the faster one on B200: D = 64 TC=1,1 one warp per domain, two cells per lane,
 // warp-level synchronisation only; TC=2,2 at D = 64 two domains per warp; D = 128 four warps with two cells per lane), variant B
 // the alternative work split of the two headline shapes.  BATCH (many lattices per launch) is built for the
-// small-lattice shapes (D <= 64), where one lattice cannot fill the GPU.
+// small-lattice shapes (D <= 64, and D = 128 TC=1,1: BASELINE config 2 runs its ensembles at L = 1024 with D = 128), where one
+// lattice cannot fill the GPU.
 template <int LD, int TX, int TY, int BLK, int G, int DPB>
 SweepLaunch make_links_launch(bool dead)
 {
     using SH = LinkShape<LD, TX, TY, G, DPB>;
     SweepLaunch sl{dead ? sweep_links_kernel<LD, TX, TY, BLK, G, DPB, true> : sweep_links_kernel<LD, TX, TY, BLK, G, DPB, false>,
                    nullptr, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
-    if constexpr (LD <= 6)
+    if constexpr (LD <= 6 || (LD == 7 && TX == 1 && TY == 1))
         sl.kern_batch = dead ? sweep_links_kernel<LD, TX, TY, BLK, G, DPB, true, true> : sweep_links_kernel<LD, TX, TY, BLK, G, DPB, false, true>;
     return sl;
 }

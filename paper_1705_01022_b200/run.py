@@ -6,7 +6,8 @@
 This is the driver a user of the library needs for the workloads of BASELINE.json: a growth run from the flat state
 (p = 1, q = 0) that records the roughness W^2(t) (Eq. (3) :61), the mean height, and -- after a waiting-time
 snapshot at t = s (:80) -- the aging autocorrelations C_h(t,s) (Eq. (6) :92-98) and C_s(t,s) (:85-88); all sums of one
-measurement point come from ONE pass over the lattice (oct_observe).  `--seeds N` runs an ensemble of N independent
+measurement point come from ONE pass over the lattice (oct_observe; oct_observe_batch for an ensemble: three launches
+per 64 members).  `--seeds N` runs an ensemble of N independent
 lattices in the same kernel launches (oct_sweep_batch; the paper's curves are means over n = 20 ... 4367 runs, :200,
 :232, :248) and reports mean +- s.e.m.  Effective exponents follow Eq. (8) :108-112 between consecutive grid points,
 e_eff = ln(E(t)/E(t')) / ln(t/t') (2 beta_eff from W^2, -lambda/z from C), with propagated 1-sigma errors (Fig. 6
@@ -121,7 +122,7 @@ def simulate(L, mcs, snap, p, q, code, seeds, per_decade=8, device="cuda:0", pro
     if snap:
         grid = sorted(set(grid) | {snap} | {snap + t for t in log_grid(mcs - snap, per_decade) if snap + t <= mcs})
     sims = [binding.Sim(L, sd, device=device) for sd in seeds]
-    outs = [torch.empty(16, dtype=torch.int64, device=sims[0].device) for _ in sims]
+    outs = torch.empty((len(sims), 16), dtype=torch.int64, device=sims[0].device)     # member i's sums in row i
     snaps = [None] * len(sims)
     rows = [[] for _ in sims]
     groups = member_groups(len(sims), L, n_groups)
@@ -136,16 +137,16 @@ def simulate(L, mcs, snap, p, q, code, seeds, per_decade=8, device="cuda:0", pro
             else:
                 binding.oct_sweep_batch([sims[i] for i in members], t - t_now, p, q, code, stream=stream)
         for members, stream in zip(groups, streams):
-            for i in members:
-                if snap and t == snap:
+            if snap and t == snap:
+                for i in members:
                     snaps[i] = sims[i].oct_snapshot(stream=stream)
-                if snaps[i] is not None:
-                    sims[i].oct_observe(binding.OCT_OBS_W2 | binding.OCT_OBS_CH | binding.OCT_OBS_CS, snaps[i][0], snaps[i][1], outs[i], stream=stream)
-                else:
-                    sims[i].oct_observe(binding.OCT_OBS_W2, None, None, outs[i], stream=stream)
+            aged = snaps[members[0]] is not None
+            what = (binding.OCT_OBS_W2 | binding.OCT_OBS_CH | binding.OCT_OBS_CS) if aged else binding.OCT_OBS_W2
+            binding.oct_observe_batch([sims[i] for i in members], what, [snaps[i][0] for i in members] if aged else None,
+                                      [snaps[i][1] for i in members] if aged else None, outs[members[0]:members[-1] + 1], stream=stream)
         t_now = t
         torch.cuda.synchronize()                                 # every group has delivered its sums
-        host = torch.stack(outs).cpu().numpy()                   # one read-back per grid point
+        host = outs.cpu().numpy()                                # one read-back per grid point
         for i in range(len(sims)):
             o = [int(v) for v in host[i]]
             row = {"sweeps": t, "t": t * dt, "w2": binding.oct_w2_from_sums(L, o[0], o[1]), "mean_h": o[2] + o[0] / N, "net": o[3]}

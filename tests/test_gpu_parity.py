@@ -332,3 +332,34 @@ def test_one_pass_observables_equal_the_three_separate_calls_and_the_oracle(L):
     sim.oct_fetch(sim.oct_observe(7, snap, anchor), host.ctypes.data, 128)
     assert tuple(host[:4]) == want[1] and tuple(host[9:15]) == want[4]
     sim.close(); orc.close(); osn.close()
+
+
+def test_batch_observables_equal_the_single_calls_and_the_oracle():
+    """oct_observe_batch (one launch set for an ensemble, PAPER.md:200 / :232 sample sizes) gives every member exactly the sums
+    its own oct_observe gives, which are the oracle's; more members than one launch holds, and every `what`."""
+    L, n = 256, 67
+    code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6)
+    sims = [binding.Sim(L, 100 + i) for i in range(n)]
+    binding.oct_sweep_batch(sims, 3, 1.0, 0.0, code)
+    snaps = [s.oct_snapshot() for s in sims]
+    binding.oct_sweep_batch(sims, 2, 1.0, 0.0, code)
+    for what in (1, 2, 4, 7):
+        need = what & 6
+        got = binding.oct_observe_batch(sims, what, [sn[0] for sn in snaps] if need else None,
+                                        [sn[1] for sn in snaps] if what & 2 else None).cpu().numpy()
+        for i in (0, 1, 63, 64, n - 1):
+            one = sims[i].oct_observe(what, snaps[i][0] if need else None, snaps[i][1] if what & 2 else None).cpu().numpy()
+            assert (got[i] == one).all(), (what, i)
+    for i in (0, 65):
+        o = Oracle(L, 100 + i)
+        o.sweep(3, 1.0, 0.0, code)
+        osnap = o.clone()
+        o.sweep(2, 1.0, 0.0, code)
+        assert tuple(int(v) for v in got[i][:4]) == o.sums()
+        assert tuple(int(v) for v in got[i][4:9]) == o.autocorr_sums(osnap)
+        assert tuple(int(v) for v in got[i][9:15]) == o.slope_autocorr_sums(osnap)
+        o.close(); osnap.close()
+    with pytest.raises(binding.OctError):
+        binding.oct_observe_batch(sims, 2, None, None)
+    for s in sims:
+        s.close()
