@@ -79,7 +79,7 @@ enum { OCT_BLK_DB = 0, OCT_BLK_DB_DELAYED = 1, OCT_BLK_DT = 2, OCT_BLK_DTR = 3 }
 
 /* Sizes of the caller-allocated device buffers for an L x L lattice (0 if L is invalid). */
 size_t oct_lattice_bytes(uint32_t L);      /* L*L/4                                                  */
-size_t oct_workspace_bytes(uint32_t L);    /* 256 + 10 L: counters, two arrays of row anchors, column scratch */
+size_t oct_workspace_bytes(uint32_t L);    /* 1280 + 10 L: counters, two arrays of row anchors, column scratch */
 
 /* Create a simulation on caller-owned device buffers (both 16-byte aligned).  Problem statement:
  * Sec. 2.1 :25-34 (model), :127 (periodic, L x L).  L must be a power of two, 16 <= L <= 2^17.

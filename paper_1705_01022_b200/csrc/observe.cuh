@@ -14,81 +14,98 @@ namespace octb {
 
 // ---- kernel 1: anchor[y] = sum_{j=1..y} sigma_y(0,j) -----------------------------------------------------
 // sigma_y(0, 4wy+j) is bit 8j+1 of word (wx=0, wy).  Column 0 is strided by one lattice row per word: L/4 separate
-// 32-byte sectors.  One SM cannot keep enough of them in flight (a single CTA doing the strided reads took 25 us at
-// L = 2^16, a tenth of the W^2 pass it precedes; profiles/r2_observables.md), so the column is first gathered into a compact
-// array by a grid of CTAs (column_gather_kernel) and then scanned by one CTA per lattice from coalesced loads.
-constexpr int kGatherThreads = 256;
+// 32-byte sectors.  One SM cannot keep enough of them in flight (a single CTA doing the strided reads and the scan took
+// 25 us at L = 2^16, a tenth of the W^2 pass it precedes; profiles/r2_observables.md), so the pass is two grids of CTAs of
+// kColThreads words each: column_gather_kernel copies the column into a compact array and leaves every CTA's net slope
+// in blocksum[]; column_anchor_kernel scans its own words and adds the sums of the CTAs before it.
+constexpr int kColThreads = 256;
+constexpr int kColMaxBlocks = 128;     // L <= 2^17: 2^15 words in column 0
 
-// col[k][w] = lat_k[w * LW] for the lattices k = blockIdx.y (one or two: current lattice and snapshot)
-__global__ void __launch_bounds__(kGatherThreads)
-column_gather_kernel(const uint32_t* __restrict__ lat0, const uint32_t* __restrict__ lat1, uint32_t L,
-                     uint32_t* __restrict__ col0, uint32_t* __restrict__ col1)
+__device__ __forceinline__ int word_dy(uint32_t v) { return 2 * __popc(v & 0x02020202u) - 4; }   // net sigma_y of the word's first column
+
+__device__ __forceinline__ void column_gather_body(const uint32_t* __restrict__ lat, uint32_t L, uint32_t* __restrict__ col,
+                                                   int32_t* __restrict__ blocksum)
 {
+    __shared__ int32_t wsum[kColThreads / 32];
     const uint32_t LW = L >> 2;
-    const uint32_t w = blockIdx.x * kGatherThreads + threadIdx.x;
-    const uint32_t* lat = blockIdx.y ? lat1 : lat0;
-    uint32_t* col = blockIdx.y ? col1 : col0;
-    if (w < LW) col[w] = lat[(size_t)w * LW];
-}
-
-constexpr int kAnchorThreads = 1024;
-
-constexpr int kAnchorMaxPer = 32;      // L <= 2^17: at most 2^15 words in column 0 = 32 per thread
-
-// inclusive scan of one gathered column by one CTA; also clears the n_zero output words of the reduction that follows
-// (this kernel precedes it in the stream: no separate memset)
-__device__ __forceinline__ void column_anchor_body(const uint32_t* __restrict__ col, uint32_t L, int32_t* __restrict__ anchor,
-                                                   unsigned long long* __restrict__ zero, int n_zero)
-{
-    __shared__ int32_t part[kAnchorThreads];
-    if ((int)threadIdx.x < n_zero) zero[threadIdx.x] = 0ull;
-    const uint32_t LW = L >> 2;
-    const uint32_t per = (LW + kAnchorThreads - 1) / kAnchorThreads;     // words of column 0 per thread
-    const uint32_t w0 = threadIdx.x * per;
-    uint32_t v[kAnchorMaxPer];
-#pragma unroll
-    for (int k = 0; k < kAnchorMaxPer; ++k) {
-        const uint32_t w = w0 + k;
-        v[k] = ((uint32_t)k < per && w < LW) ? col[w] : 0u;
+    const uint32_t w = blockIdx.x * kColThreads + threadIdx.x;
+    int s = 0;
+    if (w < LW) {
+        const uint32_t v = lat[(size_t)w * LW];
+        col[w] = v;
+        s = word_dy(v);
     }
-    int32_t sum = 0;
-#pragma unroll
-    for (int k = 0; k < kAnchorMaxPer; ++k)
-        if ((uint32_t)k < per && w0 + k < LW) sum += 2 * __popc(v[k] & 0x02020202u) - 4;
-    part[threadIdx.x] = sum;
+    s = __reduce_add_sync(0xFFFFFFFFu, s);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = s;
     __syncthreads();
-    // inclusive Hillis-Steele scan over the per-thread totals
-    for (int off = 1; off < kAnchorThreads; off <<= 1) {
-        int32_t u = threadIdx.x >= (unsigned)off ? part[threadIdx.x - off] : 0;
-        __syncthreads();
-        part[threadIdx.x] += u;
-        __syncthreads();
-    }
-    // running value entering this thread's first word.  The scan counts sigma_y(0,0) as well, which closes the
-    // loop around the torus and is not part of the path from (0,0); remove it.
-    const int32_t s00 = (col[0] >> 1) & 1u ? 1 : -1;
-    int32_t run = part[threadIdx.x] - sum - s00;
+    if (threadIdx.x == 0) {
+        int t = 0;
 #pragma unroll
-    for (int k = 0; k < kAnchorMaxPer; ++k) {
-        const uint32_t w = w0 + k;
-        if ((uint32_t)k < per && w < LW) {
-            int32_t a[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                run += (v[k] >> (8 * j + 1)) & 1u ? 1 : -1;
-                a[j] = run;
-            }
-            *reinterpret_cast<int4*>(anchor + 4 * w) = make_int4(a[0], a[1], a[2], a[3]);
-        }
+        for (int k = 0; k < kColThreads / 32; ++k) t += wsum[k];
+        blocksum[blockIdx.x] = t;
     }
 }
 
-// one CTA per lattice (blockIdx.x: 0 current lattice, 1 snapshot)
-__global__ void __launch_bounds__(kAnchorThreads)
-column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restrict__ col1, uint32_t L,
+// anchors of the words of CTA blockIdx.x; also clears the n_zero output words of the reduction that follows (this kernel
+// precedes it in the stream: no separate memset)
+__device__ __forceinline__ void column_anchor_body(const uint32_t* __restrict__ col, const int32_t* __restrict__ blocksum, uint32_t L,
+                                                   int32_t* __restrict__ anchor, unsigned long long* __restrict__ zero, int n_zero)
+{
+    __shared__ int32_t wtot[kColThreads / 32];
+    __shared__ int32_t base;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (blockIdx.x == 0 && (int)threadIdx.x < n_zero) zero[threadIdx.x] = 0ull;
+    const uint32_t LW = L >> 2;
+    const uint32_t w = blockIdx.x * kColThreads + threadIdx.x;
+    const uint32_t v = w < LW ? col[w] : 0x02020000u;                 // zero net slope past the end
+    const int s = word_dy(v);
+    int incl = s;                                                     // inclusive scan inside the warp
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const int u = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+        if (lane >= off) incl += u;
+    }
+    if (lane == 31) wtot[warp] = incl;
+    if (warp == 0) {
+        // net slope of the CTAs before this one.  The scan counts sigma_y(0,0) as well, which closes the loop around the
+        // torus and is not part of the path from (0,0); remove it.
+        int t = 0;
+#pragma unroll
+        for (int k = 0; k < kColMaxBlocks / 32; ++k) {
+            const uint32_t bidx = (uint32_t)(lane + 32 * k);
+            if (bidx < blockIdx.x) t += blocksum[bidx];
+        }
+        t = __reduce_add_sync(0xFFFFFFFFu, t);
+        if (lane == 0) base = t - ((col[0] >> 1) & 1u ? 1 : -1);
+    }
+    __syncthreads();
+    int run = base + incl - s;                                        // value entering this thread's word
+    for (int k = 0; k < warp; ++k) run += wtot[k];
+    if (w < LW) {
+        int32_t a[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            run += (v >> (8 * j + 1)) & 1u ? 1 : -1;
+            a[j] = run;
+        }
+        *reinterpret_cast<int4*>(anchor + 4 * w) = make_int4(a[0], a[1], a[2], a[3]);
+    }
+}
+
+// the lattices k = blockIdx.y (one or two: current lattice and snapshot)
+__global__ void __launch_bounds__(kColThreads)
+column_gather_kernel(const uint32_t* __restrict__ lat0, const uint32_t* __restrict__ lat1, uint32_t L,
+                     uint32_t* __restrict__ col0, uint32_t* __restrict__ col1, int32_t* __restrict__ blocksum)
+{
+    column_gather_body(blockIdx.y ? lat1 : lat0, L, blockIdx.y ? col1 : col0, blocksum + blockIdx.y * kColMaxBlocks);
+}
+
+__global__ void __launch_bounds__(kColThreads)
+column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restrict__ col1, const int32_t* __restrict__ blocksum, uint32_t L,
                      int32_t* __restrict__ anchor0, int32_t* __restrict__ anchor1, unsigned long long* __restrict__ zero, int n_zero)
 {
-    column_anchor_body(blockIdx.x ? col1 : col0, L, blockIdx.x ? anchor1 : anchor0, zero, blockIdx.x ? 0 : n_zero);
+    column_anchor_body(blockIdx.y ? col1 : col0, blocksum + blockIdx.y * kColMaxBlocks, L, blockIdx.y ? anchor1 : anchor0, zero,
+                       blockIdx.y ? 0 : n_zero);
 }
 
 // ---- kernel 2 -------------------------------------------------------------------------------------
@@ -114,6 +131,7 @@ struct ObsMember {
     int32_t* anchorB;
     uint32_t* colA;
     uint32_t* colB;
+    int32_t* blocksum;                      // 2 x kColMaxBlocks
     const unsigned long long* countersA;
     const long long* snapB;
     unsigned long long* out;                // 16 int64 of this member
@@ -124,20 +142,17 @@ struct ObsBatchParams {
     ObsMember m[kMaxObsBatch];
 };
 
-__global__ void __launch_bounds__(kGatherThreads) column_gather_batch_kernel(const __grid_constant__ ObsBatchParams BP)
+__global__ void __launch_bounds__(kColThreads) column_gather_batch_kernel(const __grid_constant__ ObsBatchParams BP)
 {
     const ObsMember& mb = BP.m[blockIdx.z];
-    const uint32_t LW = BP.L >> 2;
-    const uint32_t w = blockIdx.x * kGatherThreads + threadIdx.x;
-    const uint32_t* lat = blockIdx.y ? mb.latB : mb.latA;
-    uint32_t* col = blockIdx.y ? mb.colB : mb.colA;
-    if (w < LW) col[w] = lat[(size_t)w * LW];
+    column_gather_body(blockIdx.y ? mb.latB : mb.latA, BP.L, blockIdx.y ? mb.colB : mb.colA, mb.blocksum + blockIdx.y * kColMaxBlocks);
 }
 
-__global__ void __launch_bounds__(kAnchorThreads) column_anchor_batch_kernel(const __grid_constant__ ObsBatchParams BP)
+__global__ void __launch_bounds__(kColThreads) column_anchor_batch_kernel(const __grid_constant__ ObsBatchParams BP)
 {
-    const ObsMember& mb = BP.m[blockIdx.y];
-    column_anchor_body(blockIdx.x ? mb.colB : mb.colA, BP.L, blockIdx.x ? mb.anchorB : mb.anchorA, mb.out, blockIdx.x ? 0 : BP.n_zero);
+    const ObsMember& mb = BP.m[blockIdx.z];
+    column_anchor_body(blockIdx.y ? mb.colB : mb.colA, mb.blocksum + blockIdx.y * kColMaxBlocks, BP.L, blockIdx.y ? mb.anchorB : mb.anchorA,
+                       mb.out, blockIdx.y ? 0 : BP.n_zero);
 }
 
 // ---- slope (lattice-gas) autocorrelation C_s(t,s), PAPER.md:85-88 --------------------------------------

@@ -18,6 +18,8 @@
 
 using namespace octb;
 
+constexpr size_t kWsHeader = 256 + 2 * kColMaxBlocks * sizeof(int32_t);
+
 struct oct_ctx {
     uint32_t L = 0, log2L = 0;
     uint64_t seed = 0;
@@ -33,10 +35,12 @@ struct oct_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 
     unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws); }
-    int32_t* anchorA() const { return reinterpret_cast<int32_t*>(ws + 256); }
-    int32_t* anchorB() const { return reinterpret_cast<int32_t*>(ws + 256 + (size_t)L * 4); }
-    uint32_t* colA() const { return reinterpret_cast<uint32_t*>(ws + 256 + (size_t)L * 8); }          // column 0, gathered (L/4 words)
-    uint32_t* colB() const { return reinterpret_cast<uint32_t*>(ws + 256 + (size_t)L * 9); }
+    // workspace: [0, 16) counters; [256, 1280) net slope of every CTA's part of column 0 (two lattices); then the arrays
+    int32_t* blocksum() const { return reinterpret_cast<int32_t*>(ws + 256); }
+    int32_t* anchorA() const { return reinterpret_cast<int32_t*>(ws + kWsHeader); }
+    int32_t* anchorB() const { return reinterpret_cast<int32_t*>(ws + kWsHeader + (size_t)L * 4); }
+    uint32_t* colA() const { return reinterpret_cast<uint32_t*>(ws + kWsHeader + (size_t)L * 8); }    // column 0, gathered (L/4 words)
+    uint32_t* colB() const { return reinterpret_cast<uint32_t*>(ws + kWsHeader + (size_t)L * 9); }
 };
 
 namespace {
@@ -189,9 +193,10 @@ void launch_rows(int what, const RowsParams& rp, uint32_t LW, cudaStream_t st)
 int launch_anchors(oct_ctx* c, const uint32_t* latB, cudaStream_t st, void* zero = nullptr, int n_zero = 0)
 {
     const uint32_t LW = c->L >> 2, nlat = latB ? 2u : 1u;
-    column_gather_kernel<<<dim3((LW + kGatherThreads - 1) / kGatherThreads, nlat), kGatherThreads, 0, st>>>(c->lat, latB, c->L, c->colA(), c->colB());
-    column_anchor_kernel<<<nlat, kAnchorThreads, 0, st>>>(c->colA(), c->colB(), c->L, c->anchorA(), c->anchorB(),
-                                                         static_cast<unsigned long long*>(zero), n_zero);
+    const dim3 grid((LW + kColThreads - 1) / kColThreads, nlat);
+    column_gather_kernel<<<grid, kColThreads, 0, st>>>(c->lat, latB, c->L, c->colA(), c->colB(), c->blocksum());
+    column_anchor_kernel<<<grid, kColThreads, 0, st>>>(c->colA(), c->colB(), c->blocksum(), c->L, c->anchorA(), c->anchorB(),
+                                                      static_cast<unsigned long long*>(zero), n_zero);
     c->launches += 2;
     OCT_CUDA(c, cudaGetLastError());
     return OCT_OK;
@@ -203,7 +208,7 @@ extern "C" {
 
 size_t oct_lattice_bytes(uint32_t L) { return valid_L(L) ? (size_t)L * L / 4 : 0; }
 
-size_t oct_workspace_bytes(uint32_t L) { return valid_L(L) ? 256 + 10 * (size_t)L : 0; }   // counters; 2 x L int32 anchors; 2 x L/4 words of column 0
+size_t oct_workspace_bytes(uint32_t L) { return valid_L(L) ? kWsHeader + 10 * (size_t)L : 0; }   // header; 2 x L int32 anchors; 2 x L/4 words of column 0
 
 int oct_create(oct_ctx** out, uint32_t L, uint64_t seed, int init, void* lattice_dev, void* workspace_dev, void* stream)
 {
@@ -548,15 +553,16 @@ int oct_observe_batch(oct_ctx* const* cs, uint32_t n, int what, const void* cons
             const oct_ctx* c = cs[m0 + m];
             ObsMember& mb = bp.m[m];
             mb.latA = c->lat; mb.latB = need_snap ? static_cast<const uint32_t*>(snapshots_dev[m0 + m]) : nullptr;
-            mb.anchorA = c->anchorA(); mb.anchorB = c->anchorB(); mb.colA = c->colA(); mb.colB = c->colB();
+            mb.anchorA = c->anchorA(); mb.anchorB = c->anchorB(); mb.colA = c->colA(); mb.colB = c->colB(); mb.blocksum = c->blocksum();
             mb.countersA = c->counters();
             mb.snapB = (what & OCT_OBS_CH) ? reinterpret_cast<const long long*>(snapshot_anchors_dev[m0 + m]) : nullptr;
             mb.out = reinterpret_cast<unsigned long long*>(out_dev) + (size_t)(m0 + m) * 16;
         }
         if (need_anchor) {
             const uint32_t nlat = (what & OCT_OBS_CH) ? 2u : 1u;
-            column_gather_batch_kernel<<<dim3((LW + kGatherThreads - 1) / kGatherThreads, nlat, nb), kGatherThreads, 0, st>>>(bp);
-            column_anchor_batch_kernel<<<dim3(nlat, nb), kAnchorThreads, 0, st>>>(bp);
+            const dim3 grid((LW + kColThreads - 1) / kColThreads, nlat, nb);
+            column_gather_batch_kernel<<<grid, kColThreads, 0, st>>>(bp);
+            column_anchor_batch_kernel<<<grid, kColThreads, 0, st>>>(bp);
             c0->launches += 2;
         }
         launch_rows_batch(what, bp, nb, LW, st);

@@ -30,7 +30,7 @@ def test_library_exports_every_declared_symbol():
 def test_sizes_and_L_validation():
     assert binding.oct_lattice_bytes(256) == 256 * 256 // 4
     assert binding.oct_lattice_bytes(1 << 17) == 1 << 32
-    assert binding.oct_workspace_bytes(256) == 256 + 10 * 256
+    assert binding.oct_workspace_bytes(256) == 1280 + 10 * 256
     for bad in (0, 8, 100, 3 << 10, 1 << 18):
         assert binding.oct_lattice_bytes(bad) == 0 and binding.oct_workspace_bytes(bad) == 0
 
