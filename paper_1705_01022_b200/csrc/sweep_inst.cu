@@ -52,38 +52,38 @@ bool OCT_CAT(oct_find_packed_, OCT_INST_LOG2D)(int tx, int ty, int blk, SweepLau
 }
 
 #else
-// ---- link-entry kernel: (log2 D, tcx, tcy, threads per domain, domains per CTA) -------------------------
+// ---- link-entry kernel: (log2 D, tcx, tcy, threads per domain, domains per CTA, bytes per entry) ----------
 // Variant A is the default (the faster one on B200: D = 64 TC=1,1 one warp per domain, two cells per lane,
 // warp-level synchronisation only; TC=2,2 at D = 64 two domains per warp; D = 128 four warps with two cells per lane), variant B
 // the alternative work split of the two headline shapes.  BATCH (many lattices per launch) is built for the
 // small-lattice shapes (D <= 64, and D = 128 TC=1,1: BASELINE config 2 runs its ensembles at L = 1024 with D = 128), where one
 // lattice cannot fill the GPU.
-template <int LD, int TX, int TY, int BLK, int G, int DPB>
+template <int LD, int TX, int TY, int BLK, int G, int DPB, int EB>
 SweepLaunch make_links_launch(bool dead)
 {
-    using SH = LinkShape<LD, TX, TY, G, DPB>;
-    SweepLaunch sl{dead ? sweep_links_kernel<LD, TX, TY, BLK, G, DPB, true> : sweep_links_kernel<LD, TX, TY, BLK, G, DPB, false>,
+    using SH = LinkShape<LD, TX, TY, G, DPB, EB>;
+    SweepLaunch sl{dead ? sweep_links_kernel<LD, TX, TY, BLK, G, DPB, true, false, EB> : sweep_links_kernel<LD, TX, TY, BLK, G, DPB, false, false, EB>,
                    nullptr, SH::NTHREADS, SH::SMEM_BYTES, SH::DPB};
     if constexpr (LD <= 6 || (LD == 7 && TX == 1 && TY == 1))
-        sl.kern_batch = dead ? sweep_links_kernel<LD, TX, TY, BLK, G, DPB, true, true> : sweep_links_kernel<LD, TX, TY, BLK, G, DPB, false, true>;
+        sl.kern_batch = dead ? sweep_links_kernel<LD, TX, TY, BLK, G, DPB, true, true, EB> : sweep_links_kernel<LD, TX, TY, BLK, G, DPB, false, true, EB>;
     return sl;
 }
 
-#define OCT_LINK_SHAPES_A_5(X) X(5, 0, 0, 32, 4) X(5, 1, 1, 16, 8)
-#define OCT_LINK_SHAPES_A_6(X) X(6, 0, 0, 128, 1) X(6, 1, 1, 32, 4) X(6, 2, 1, 32, 4) X(6, 2, 2, 16, 2)
-#define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1) X(7, 1, 1, 128, 1) X(7, 2, 2, 64, 1) X(7, 2, 1, 128, 1) X(7, 3, 2, 32, 1) X(7, 4, 1, 32, 1)
+#define OCT_LINK_SHAPES_A_5(X) X(5, 0, 0, 32, 4, 4) X(5, 1, 1, 16, 8, 4)
+#define OCT_LINK_SHAPES_A_6(X) X(6, 0, 0, 128, 1, 4) X(6, 1, 1, 32, 4, 4) X(6, 2, 1, 32, 4, 4) X(6, 2, 2, 16, 4, 2)
+#define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1, 4) X(7, 1, 1, 128, 1, 4) X(7, 2, 2, 64, 1, 4) X(7, 2, 1, 128, 1, 4) X(7, 3, 2, 32, 1, 4) X(7, 4, 1, 32, 1, 4)
 #define OCT_LINK_SHAPES_B_5(X)
-#define OCT_LINK_SHAPES_B_6(X) X(6, 1, 1, 64, 2)
-#define OCT_LINK_SHAPES_B_7(X) X(7, 1, 1, 256, 1)
+#define OCT_LINK_SHAPES_B_6(X) X(6, 1, 1, 64, 2, 4) X(6, 2, 2, 16, 2, 4)
+#define OCT_LINK_SHAPES_B_7(X) X(7, 1, 1, 256, 1, 4)
 
 bool OCT_CAT(oct_find_links_, OCT_INST_LOG2D)(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out)
 {
-#define X(LD, TX, TY, G, DPB)                                                                        \
+#define X(LD, TX, TY, G, DPB, EB)                                                                    \
     if (tx == TX && ty == TY) {                                                                      \
-        if (blk == kBlkSync) { *out = make_links_launch<LD, TX, TY, kBlkSync, G, DPB>(dead); return true; }       \
-        if (blk == kBlkDelayed) { *out = make_links_launch<LD, TX, TY, kBlkDelayed, G, DPB>(dead); return true; } \
+        if (blk == kBlkSync) { *out = make_links_launch<LD, TX, TY, kBlkSync, G, DPB, EB>(dead); return true; }       \
+        if (blk == kBlkDelayed) { *out = make_links_launch<LD, TX, TY, kBlkDelayed, G, DPB, EB>(dead); return true; } \
         if constexpr (TX >= 1 && TY >= 1) {                                                          \
-            if (blk == kBlkDT) { *out = make_links_launch<LD, TX, TY, kBlkDT, G, DPB>(dead); return true; }       \
+            if (blk == kBlkDT) { *out = make_links_launch<LD, TX, TY, kBlkDT, G, DPB, EB>(dead); return true; }       \
         }                                                                                            \
         return false;                                                                                \
     }

@@ -37,12 +37,20 @@ namespace octb {
 
 constexpr uint32_t kEntryMin = 0xFF00FF00u;   // (W,E,S,N) = (0,1,0,1): local minimum, Eq. (1); a set link is the byte 0xFF
 constexpr uint32_t kEntryMax = 0x00FF00FFu;   // (1,0,1,0): local maximum
+// Two-byte entries (EB = 2): a site keeps only its OWN links (W, S); the test gathers (W, S, E, N) from three loads --
+// the entry, the east neighbour's W byte, the north neighbour's S byte -- and an update is three stores.  Half the shared
+// memory per domain, i.e. twice the domains in flight: for shapes with few cells per domain (TC=2,2: 16 cells per 64 x 64
+// domain), which are bound by the latency of the step chain, not by the shared-memory pipe (profiles/r2_sweep.md).
+constexpr uint32_t kEntry2Min = 0xFFFF0000u;  // (W,S,E,N) = (0,0,1,1)
+constexpr uint32_t kEntry2Max = 0x0000FFFFu;
 
 // G_ = threads of the worker group that owns one domain: a multiple of 32 (one or several warps), or 16 -- two
 // domains per warp, for domains with only 16 thread cells (TC=2,2 at D = 64: the paper's second production
 // configuration, Fig. 5 :236-244).  DPB_ = domains per CTA.
-template <int LOG2D, int TCX, int TCY, int G_, int DPB_>
+template <int LOG2D, int TCX, int TCY, int G_, int DPB_, int EB_ = 4>
 struct LinkShape {
+    static constexpr int EB = EB_;                        // bytes per entry: 4 (W,E,S,N) or 2 (W,S)
+    static_assert(EB == 4 || EB == 2, "entries are four or two link bytes");
     static constexpr int D = 1 << LOG2D;
     static constexpr int CX = 4 << TCX, CY = 4 << TCY;
     static constexpr int NCX = D / CX, NCY = D / CY, NCELL = NCX * NCY;
@@ -52,8 +60,8 @@ struct LinkShape {
     static constexpr int NTHREADS = G * DPB;
     static constexpr int NW = D / 4 + 1;                  // window edge in packed words (halo included)
     static constexpr int P = 4 * NW;                      // entries per row (multiple of 4: 128-bit rows)
-    static constexpr int ROWS = 4 * NW + 1;               // one spare row below row 0 for stray S-writes
-    static constexpr int ENTRY_WORDS = ROWS * P;
+    static constexpr int ROWS = EB == 4 ? 4 * NW + 1 : 4 * NW;   // four-byte entries: one spare row below row 0 for stray S-writes
+    static constexpr int ENTRY_WORDS = ROWS * P * EB / 4;
     // block-step words (one per collective step, R13/R17) are kept in shared memory for BTW steps at a time; two
     // domains per warp keep 16 only, so that six CTAs of two domains fit one SM (6 x (2 x 18832 + 1024) B <= 228 KiB)
     static constexpr int BTW = (G_ == 16 && NSTEP > 64) ? 16 : (NSTEP < 64 ? NSTEP : 64);
@@ -68,6 +76,7 @@ struct LinkShape {
 #define OCT_LINKS_FAST_STAGE 1
 #endif
     static constexpr bool FAST_17 = (OCT_LINKS_FAST_STAGE && (G == 32 || G == 16) && NW == 17);
+    static_assert(ENTRY_WORDS % 4 == 0, "the block-step ring behind the entries is read with 128-bit loads");
     static_assert(CX <= D && CY <= D, "cell larger than domain");
 };
 
@@ -88,6 +97,27 @@ template <class SH>
 __device__ __forceinline__ void expand_word(uint32_t* __restrict__ S, uint32_t iw, uint32_t jw, uint32_t A,
                                             uint32_t Ew, uint32_t Nw)
 {
+    if constexpr (SH::EB == 2) {
+        // two-byte entries: the 8 bytes of a site row are its 8 packed bits in order (W0, S0, W1, S1, ...), sign-replicated
+        // from shifted copies: bit k of every row at the top of the bytes of A << (7 - k); no neighbour words needed
+        uint32_t T[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) T[k] = A << (7 - k);
+        uint32_t p01[4], p23[4];                                  // bits (2q, 2q+1) of rows 0, 1 / rows 2, 3
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            p01[q] = prmt(T[2 * q], T[2 * q + 1], 0xD9C8u);
+            p23[q] = prmt(T[2 * q], T[2 * q + 1], 0xFBEAu);
+        }
+        unsigned short* E = reinterpret_cast<unsigned short*>(S);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t (&pp)[4] = j < 2 ? p01 : p23;
+            const uint32_t sel = (j & 1) ? 0x7632u : 0x5410u;
+            *reinterpret_cast<uint2*>(E + (4 * jw + j) * SH::P + 4 * iw) = make_uint2(prmt(pp[0], pp[1], sel), prmt(pp[2], pp[3], sel));
+        }
+        return;
+    }
     uint32_t BW[5], BS[4], BN[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -118,6 +148,7 @@ template <class SH>
 __device__ __forceinline__ void expand_word_rot(uint32_t* __restrict__ S, uint32_t iw, uint32_t jw, uint32_t A,
                                                 uint32_t Ew, uint32_t Nw, uint32_t rot)
 {
+    if constexpr (SH::EB == 2) { expand_word<SH>(S, iw, jw, A, Ew, Nw); return; }   // (one word in 17: the conflicts do not matter)
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const uint32_t jj = ((uint32_t)j + rot) & 3u;
@@ -149,14 +180,21 @@ __device__ __forceinline__ uint32_t gather_word(const uint32_t* __restrict__ S, 
 {
     uint32_t p[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
-        p[j] = row_bits_top(*reinterpret_cast<const uint4*>(S + (4 * jw + j) * SH::P + 4 * iw));
+    for (int j = 0; j < 4; ++j) {
+        if constexpr (SH::EB == 2) {
+            const uint2 v = *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned short*>(S) + (4 * jw + j) * SH::P + 4 * iw);
+            p[j] = ((v.x & 0x08040201u) | (v.y & 0x80402010u)) * 0x01010101u;   // byte k keeps bit k; the multiply adds the bytes
+        } else {
+            p[j] = row_bits_top(*reinterpret_cast<const uint4*>(S + (4 * jw + j) * SH::P + 4 * iw));
+        }
+    }
     return prmt(prmt(p[0], p[1], 0x0073u), prmt(p[2], p[3], 0x0073u), 0x5410u);
 }
 
 template <class SH>
 __device__ __forceinline__ uint32_t gather_word_rot(const uint32_t* __restrict__ S, uint32_t iw, uint32_t jw, uint32_t rot)
 {
+    if constexpr (SH::EB == 2) return gather_word<SH>(S, iw, jw);
     uint32_t word = 0;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -181,6 +219,13 @@ __device__ __forceinline__ uint32_t site_index(uint32_t v, uint32_t soff)
 template <class SH>
 __device__ __forceinline__ void flip_links(uint32_t* Sb, uint32_t i, bool up)
 {
+    if constexpr (SH::EB == 2) {
+        unsigned char* B2 = reinterpret_cast<unsigned char*>(Sb) + 2u * i;
+        *reinterpret_cast<unsigned short*>(B2) = up ? 0xFFFF : 0;      // own W and S links
+        B2[2] = up ? 0 : 0xFF;                                         // east neighbour's W link = sigma_x(x+1,y)
+        B2[2 * SH::P + 1] = up ? 0 : 0xFF;                             // north neighbour's S link = sigma_y(x,y+1)
+        return;
+    }
     unsigned char* B = reinterpret_cast<unsigned char*>(Sb + i);
     const unsigned char v1 = up ? 0xFF : 0, v0 = up ? 0 : 0xFF;
     Sb[i] = up ? kEntryMax : kEntryMin;
@@ -193,12 +238,13 @@ __device__ __forceinline__ void flip_links(uint32_t* Sb, uint32_t i, bool up)
 // Acceptance rule of one launch.  ONEDIR: only one of p, q is non-zero (always so for the sync variant),
 // so a single entry pattern is tested and the stored values are launch constants; ALWAYS: that live
 // threshold is 65536 (p = 1 or q = 1) and the 16-bit comparison is dropped as well.
-template <bool ONEDIR, bool ALWAYS>
+template <bool ONEDIR, bool ALWAYS, int EB = 4>
 struct Rule {
+    static constexpr uint32_t kMin = EB == 4 ? kEntryMin : kEntry2Min, kMax = EB == 4 ? kEntryMax : kEntry2Max;
     uint32_t P16, Q16, target, T16;
     bool dep;
     __device__ __forceinline__ Rule(uint32_t p16, uint32_t q16)
-        : P16(p16), Q16(q16), target(q16 == 0u ? kEntryMin : kEntryMax), T16(q16 == 0u ? p16 : q16), dep(q16 == 0u) {}
+        : P16(p16), Q16(q16), target(q16 == 0u ? kMin : kMax), T16(q16 == 0u ? p16 : q16), dep(q16 == 0u) {}
     // decision for entry value e and attempt word w: 0 nothing, +1 deposit, -1 remove
     __device__ __forceinline__ int decide(uint32_t e, uint32_t w) const
     {
@@ -208,7 +254,7 @@ struct Rule {
             return acc ? (dep ? 1 : -1) : 0;
         } else {
             const uint32_t r16 = w >> 16;
-            return (e == kEntryMin && r16 < P16) ? 1 : ((e == kEntryMax && r16 < Q16) ? -1 : 0);
+            return (e == kMin && r16 < P16) ? 1 : ((e == kMax && r16 < Q16) ? -1 : 0);
         }
     }
     // carry out decision d at entry i and count it in net (deposits - removals; ONEDIR counts updates, the caller signs them)
@@ -256,7 +302,7 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
         const uint32_t c = tg + j * G;
         cellc[j] = ((c & (SH::NCX - 1)) * CX) | (((c >> LOG2NCX) * CY) << 8);
     }
-    const Rule<ONEDIR, ALWAYS> rule(P16, Q16);
+    const Rule<ONEDIR, ALWAYS, SH::EB> rule(P16, Q16);
 
     // decision for the site packed in v (x | y << 8 before wrapping); idx receives its entry index
     auto decide_site = [&](uint32_t v, uint32_t w, uint32_t& idx) -> int {
@@ -265,7 +311,13 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
             const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
             if ((vm & 0xFFu) >= dead_lim || (vm >> 8) >= dead_lim) return 0;      // dead border: not carried out
         }
-        return rule.decide(S[idx], w);
+        if constexpr (SH::EB == 2) {
+            const unsigned char* B2 = reinterpret_cast<const unsigned char*>(S) + 2u * idx;
+            const uint32_t own = *reinterpret_cast<const unsigned short*>(B2), ea = B2[2], no = B2[2 * SH::P + 1];
+            return rule.decide(own | (ea << 16) | (no << 24), w);          // (W, S, E, N)
+        } else {
+            return rule.decide(S[idx], w);
+        }
     };
     int net = 0;                                     // accepted updates of this lane's cells (counted under the stores' predicate)
 
@@ -365,7 +417,12 @@ template <class SH>
 __device__ __forceinline__ int row_links_up(const uint32_t* Sb, uint32_t n00, uint32_t y00, uint32_t tg)
 {
     int n = 0;
-    for (uint32_t x = tg; x < n00; x += SH::G) n += (int)(Sb[y00 * SH::P + x] & 1u);
+    if constexpr (SH::EB == 2) {       // Sb = entry (0,0) of the domain as a two-byte entry pointer
+        const unsigned char* B = reinterpret_cast<const unsigned char*>(Sb);
+        for (uint32_t x = tg; x < n00; x += SH::G) n += (int)(B[2u * (y00 * SH::P + x)] & 1u);
+    } else {
+        for (uint32_t x = tg; x < n00; x += SH::G) n += (int)(Sb[y00 * SH::P + x] & 1u);
+    }
     return n;
 }
 
@@ -375,18 +432,18 @@ __device__ __forceinline__ const SweepParams& common_params(const SweepBatchPara
 // DEAD = false: tiled device layers DTr / DT (four launches per MCS, one per domain set);
 // DEAD = true : dead-border device layers DB / cDB / DBh (all tiles in one launch; the rim of width dead_w is
 //               never updated, and words shared with the next tile are neither read, counted nor written, :166).
-template <int LOG2D, int TCX, int TCY, int BLK, int G_, int DPB, bool DEAD, bool BATCH = false>
-__global__ void __launch_bounds__(LinkShape<LOG2D, TCX, TCY, G_, DPB>::NTHREADS)
+template <int LOG2D, int TCX, int TCY, int BLK, int G_, int DPB, bool DEAD, bool BATCH = false, int EB = 4>
+__global__ void __launch_bounds__(LinkShape<LOG2D, TCX, TCY, G_, DPB, EB>::NTHREADS)
 sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, SweepBatchParams, SweepParams>::type PP)
 {
-    using SH = LinkShape<LOG2D, TCX, TCY, G_, DPB>;
+    using SH = LinkShape<LOG2D, TCX, TCY, G_, DPB, EB>;
     constexpr int D = SH::D, G = SH::G, NW = SH::NW;
 
     extern __shared__ __align__(16) uint32_t smem_raw[];
     const int grp = threadIdx.x / G;                 // worker group inside the CTA
     const uint32_t tg = threadIdx.x % G;             // thread inside the group
     uint32_t* S0 = smem_raw + grp * (SH::SMEM_PER_DOMAIN / 4);
-    uint32_t* S = S0 + SH::P;                        // row 0 of the window (one spare row below it)
+    uint32_t* S = EB == 4 ? S0 + SH::P : S0;         // row 0 of the window (four-byte entries: one spare row below it)
     uint32_t* BT = S0 + SH::ENTRY_WORDS;             // block-step words of this domain sweep
 
     // one lattice: everything comes from the parameter block (the round keys stay in the constant bank);
@@ -436,7 +493,8 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
     }
     const uint32_t offx = gx & 3u, offy = gy & 3u;
     const uint32_t LW = L >> 2, LWm = LW - 1u, wx0 = gx >> 2, wy0 = gy >> 2;
-    uint32_t* Sb = S + offy * SH::P + offx;          // entry of the domain's site (0,0)
+    // entry of the domain's site (0,0) (two-byte entries: half as many words in)
+    uint32_t* Sb = EB == 4 ? S + offy * SH::P + offx : reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned short*>(S) + offy * SH::P + offx);
     // window words this domain reads, counts and writes back: all of them, or (dead border) only those that hold no
     // site of the next tile -- the last active site's E / N links still lie inside them (:166).  The other words
     // belong to the next tile, which writes them in this same launch: they are not even loaded (zeros stand in;
@@ -471,12 +529,16 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
         C16 = (tg == 0u && kept(NW - 1, NW - 1)) ? *word_ptr(NW - 1, NW - 1) : 0u;
 #pragma unroll
         for (int jw = 0; jw < NW; ++jw) {
-            const uint32_t e1 = __shfl_down_sync(wmask, A[jw], 1, 16);
-            const uint32_t e2 = jw < 16 ? __shfl_sync(wmask, C, jw, 16) : __shfl_sync(wmask, C16, 0, 16);
+            uint32_t e1 = 0u, e2 = 0u;                 // (two-byte entries hold no neighbour links: nothing to fetch)
+            if constexpr (EB == 4) {
+                e1 = __shfl_down_sync(wmask, A[jw], 1, 16);
+                e2 = jw < 16 ? __shfl_sync(wmask, C, jw, 16) : __shfl_sync(wmask, C16, 0, 16);
+            }
             expand_word<SH>(S, iw, jw, A[jw], iw == 15u ? e2 : e1, A[jw + 1]);
         }
         // last column: lane jw expands word (16, jw), lane 0 then (16, 16); its north word is the next lane's
-        const uint32_t Cn = __shfl_down_sync(wmask, C, 1, 16), Cn15 = __shfl_sync(wmask, C16, 0, 16);
+        uint32_t Cn = 0u, Cn15 = 0u;
+        if constexpr (EB == 4) { Cn = __shfl_down_sync(wmask, C, 1, 16); Cn15 = __shfl_sync(wmask, C16, 0, 16); }
         expand_word_rot<SH>(S, NW - 1, tg, C, 0u, tg == 15u ? Cn15 : Cn, tg >> 1);
         if (tg == 0u) {
             expand_word<SH>(S, NW - 1, NW - 1, C16, 0u, 0u);
@@ -499,13 +561,17 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
 #pragma unroll
         for (int it = 0; it < NP; ++it) {
             const uint32_t jw = 2u * it + hi;
-            const uint32_t e1 = __shfl_down_sync(0xFFFFFFFFu, A[it], 1), e2 = __shfl_sync(0xFFFFFFFFu, C, jw);
-            const uint32_t Nw = __shfl_xor_sync(0xFFFFFFFFu, hi ? A[it] : A[it + 1], 16);
+            uint32_t e1 = 0u, e2 = 0u, Nw = 0u;
+            if constexpr (EB == 4) {
+                e1 = __shfl_down_sync(0xFFFFFFFFu, A[it], 1); e2 = __shfl_sync(0xFFFFFFFFu, C, jw);
+                Nw = __shfl_xor_sync(0xFFFFFFFFu, hi ? A[it] : A[it + 1], 16);
+            }
             if (jw < (uint32_t)NW) {
                 expand_word<SH>(S, iw, jw, A[it], iw == 15u ? e2 : e1, Nw);
             }
         }
-        const uint32_t Cn = __shfl_down_sync(0xFFFFFFFFu, C, 1);
+        uint32_t Cn = 0u;
+        if constexpr (EB == 4) Cn = __shfl_down_sync(0xFFFFFFFFu, C, 1);
         if (tg < (uint32_t)NW) {
             expand_word_rot<SH>(S, NW - 1, tg, C, 0u, Cn, tg >> 1);       // the east links of this column are never read
         }
@@ -521,7 +587,9 @@ sweep_links_kernel(const __grid_constant__ typename std::conditional<BATCH, Swee
                 A[it] = Ew[it] = Nw[it] = 0u;
                 if (idx < (uint32_t)(NW * NW)) {
                     const uint32_t jw = idx / NW, iw = idx - jw * NW;
-                    if constexpr (DEAD) {
+                    if constexpr (EB == 2) {          // two-byte entries: own links only
+                        if (kept(iw, jw)) A[it] = *word_ptr(iw, jw);
+                    } else if constexpr (DEAD) {
                         if (kept(iw, jw)) A[it] = *word_ptr(iw, jw);
                         if (kept(iw + 1, jw)) Ew[it] = *word_ptr(iw + 1, jw);
                         if (kept(iw, jw + 1)) Nw[it] = *word_ptr(iw, jw + 1);
