@@ -54,8 +54,10 @@ bool OCT_CAT(oct_find_packed_, OCT_INST_LOG2D)(int tx, int ty, int blk, SweepLau
 #else
 // ---- link-entry kernel: (log2 D, tcx, tcy, threads per domain, domains per CTA, bytes per entry) ----------
 // Variant A is the default (the faster one on B200: D = 64 TC=1,1 one warp per domain, two cells per lane,
-// warp-level synchronisation only; TC=2,2 at D = 64 two domains per warp; D = 128 four warps with two cells per lane), variant B
-// the alternative work split of the two headline shapes.  BATCH (many lattices per launch) is built for the
+// warp-level synchronisation only, four-byte entries; shapes with few cells per domain -- TC=2,2 (half a warp per 64 x 64
+// domain), TC=3,2 and TC=4,1 -- two-byte entries, which double the domains in flight: measured per shape, profiles/r2_sweep.md;
+// D = 128 TC=1,1 four warps with two cells per lane), variant B the alternative work split or entry size of the shapes the
+// paper's results rest on.  BATCH (many lattices per launch) is built for the
 // small-lattice shapes (D <= 64, and D = 128 TC=1,1: BASELINE config 2 runs its ensembles at L = 1024 with D = 128), where one
 // lattice cannot fill the GPU.
 template <int LD, int TX, int TY, int BLK, int G, int DPB, int EB>
@@ -71,10 +73,10 @@ SweepLaunch make_links_launch(bool dead)
 
 #define OCT_LINK_SHAPES_A_5(X) X(5, 0, 0, 32, 4, 4) X(5, 1, 1, 16, 8, 4)
 #define OCT_LINK_SHAPES_A_6(X) X(6, 0, 0, 128, 1, 4) X(6, 1, 1, 32, 4, 4) X(6, 2, 1, 32, 4, 4) X(6, 2, 2, 16, 4, 2)
-#define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1, 4) X(7, 1, 1, 128, 1, 4) X(7, 2, 2, 64, 1, 4) X(7, 2, 1, 128, 1, 4) X(7, 3, 2, 32, 1, 4) X(7, 4, 1, 32, 1, 4)
+#define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1, 4) X(7, 1, 1, 128, 1, 4) X(7, 2, 2, 64, 1, 2) X(7, 2, 1, 128, 1, 4) X(7, 3, 2, 32, 1, 2) X(7, 4, 1, 32, 1, 2)
 #define OCT_LINK_SHAPES_B_5(X)
 #define OCT_LINK_SHAPES_B_6(X) X(6, 1, 1, 64, 2, 4) X(6, 2, 2, 16, 2, 4)
-#define OCT_LINK_SHAPES_B_7(X) X(7, 1, 1, 256, 1, 4)
+#define OCT_LINK_SHAPES_B_7(X) X(7, 1, 1, 256, 1, 4) X(7, 2, 2, 64, 1, 4)
 
 bool OCT_CAT(oct_find_links_, OCT_INST_LOG2D)(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out)
 {
