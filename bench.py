@@ -34,9 +34,20 @@ UNIT = "attempts/s"
 PAPER_ATTEMPTS_PER_S = 9.0e9
 N_SM, SMSP, LANES = 148, 4, 32
 # Conflict-free minimum of shared-memory wavefronts per warp-attempt (32 update attempts) of the link-entry sweep
-# (DESIGN.md section 5.1): 1 entry load + 5 stores of an accepted update (issued whenever a lane of the warp accepts)
-# + staging 2 x (68 x 68 entries x 4 B / 128 B) per 128 warp-attempts of a 64 x 64 domain + 1/8 block-step load.
-WAVEFRONTS_MIN = 1.0 + 5.0 + 2.0 * (68 * 68 * 4 / 128.0) / 128.0 + 0.125
+# (DESIGN.md section 5.1).  Four-byte entries: 1 entry load + 5 stores of an accepted update (issued whenever a lane of the
+# warp accepts); two-byte entries (shapes with few cells per domain): 3 loads + 3 stores.  Plus staging in and out,
+# 2 x ((D+4)^2 entries x EB bytes / 128 B) per D^2/32 warp-attempts of a domain, plus 1/8 block-step load.
+TWO_BYTE_SHAPES = {(6, 2, 2), (7, 2, 2), (7, 3, 2), (7, 4, 1)}          # (log2D, tcx, tcy), as built in csrc/sweep_inst.cu
+
+
+def wavefronts_min(log2D: int, tcx: int, tcy: int, kernel_opt: int = 0) -> float:
+    eb = 2 if ((log2D, tcx, tcy) in TWO_BYTE_SHAPES and kernel_opt != 2) else 4
+    D = 1 << log2D
+    staging = 2.0 * ((D + 4) * (D + 4) * eb / 128.0) / (D * D / 32.0)
+    return 6.0 + staging + 0.125          # six loads and stores per attempt in either layout (1 + 5 or 3 + 3)
+
+
+WAVEFRONTS_MIN = wavefronts_min(6, 1, 1)
 # Algorithmic lane-instructions per attempt: Philox 40/4 = 10, site select 5, entry load +
 # compare 2, five stores + accept count 6, loop/sync 1, staging per site 6 (permute expansion 47/16, gather 34/16, loads,
 # stores and addresses).  The executed count comes from the committed ncu capture.
@@ -227,11 +238,12 @@ def roofline_block(args, L, peaks, sweep_ms, total_ms, n_sweep_launches, kernel)
     warp_attempts = attempts_per_launch / 32
     f_hz = peaks["sm_max_mhz"] * 1e6
     peak_wf = N_SM * f_hz / 1e9                                    # G wavefronts/s: one per clock per SM
-    achieved = WAVEFRONTS_MIN * warp_attempts / launch_s / 1e9
+    wf_min = wavefronts_min(args.log2D, args.tcx, args.tcy, args.kernel)
+    achieved = wf_min * warp_attempts / launch_s / 1e9
     cnt = ncu_counters(kernel, L, args.log2D, args.tcx, args.tcy, args.blk) or ncu_counters(kernel, 1 << 16, args.log2D, args.tcx, args.tcy, args.blk)
     rf = {"bound": "smem", "achieved": achieved, "peak": peak_wf, "unit": "Gwavefront/s", "frac": achieved / peak_wf,
           "traffic": None, "kernel": kernel, "avg_launch_ms": launch_s * 1e3, "attempts_per_launch": attempts_per_launch,
-          "wavefronts_per_warp_attempt_min": WAVEFRONTS_MIN,
+          "wavefronts_per_warp_attempt_min": wf_min,
           "peak_src": f"148 SM x 1 shared-memory wavefront/clk x sm_max_mhz ({peaks['src']})",
           "hbm_gbs_of_sweep": 0.5 * (1.0 + 4.0 / (1 << args.log2D)) ** 2 * attempts_per_launch / launch_s / 1e9,
           "sweep_share_of_step": sweep_ms / total_ms}
