@@ -184,7 +184,7 @@ const char* oct_last_error(const oct_ctx*);             /* text of the last CUDA
  * which kernel runs.  OCT_OPT_KERNEL: AUTO picks the link-entry kernel (one 32-bit entry of four link
  * bytes per site in shared memory, no atomics) for D <= 128 (>= 32 cells per domain) and the bit-packed kernel
  * otherwise; BITPACKED forces the latter; LINKS_B selects the alternative work split (another number of
- * warps per domain) where one is built.  EINVAL for unknown options / values. */
+ * warps per domain) or entry size (four link bytes per site instead of two, for TC=2,2) where one is built.  EINVAL for unknown options / values. */
 enum { OCT_OPT_KERNEL = 1 };
 enum { OCT_KERNEL_AUTO = 0, OCT_KERNEL_BITPACKED = 1, OCT_KERNEL_LINKS_B = 2 };
 int oct_set_option(oct_ctx*, int option, int value);
