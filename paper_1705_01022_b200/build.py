@@ -15,7 +15,7 @@ LIB = os.path.join(HERE, "liboct_b200.so")
 # domain size so that the ~200 kernel instantiations build in parallel.
 UNITS = [("oct_api", "oct_api.cu", [])] + \
         [(f"packed_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=0", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7, 8)] + \
-        [(f"links_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=1", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7)]
+        [(f"links_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=1", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7, 8)]
 HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "observe_rows.cuh", "philox.cuh", "launch.h", "sweep_inst.cu", "oct_api.cu",
            os.path.join("..", "..", "include", "oct.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

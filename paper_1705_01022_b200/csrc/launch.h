@@ -20,5 +20,6 @@ bool oct_find_packed_8(int tx, int ty, int blk, SweepLaunch* out);
 bool oct_find_links_5(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out);
 bool oct_find_links_6(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out);
 bool oct_find_links_7(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out);
+bool oct_find_links_8(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out);   // D = 256: two-byte entries only
 
 }  // namespace octb

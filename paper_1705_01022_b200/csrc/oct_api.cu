@@ -88,6 +88,7 @@ bool find_links_launch(int ld, int tx, int ty, int blk, bool variant_b, bool dea
         case 5: return oct_find_links_5(tx, ty, blk, variant_b, dead, out);
         case 6: return oct_find_links_6(tx, ty, blk, variant_b, dead, out);
         case 7: return oct_find_links_7(tx, ty, blk, variant_b, dead, out);
+        case 8: return oct_find_links_8(tx, ty, blk, variant_b, dead, out);
         default: return false;
     }
 }

@@ -1,6 +1,6 @@
 // Instantiations of the sweep kernels.  Compiled once per (family, log2 D):
 //     -DOCT_INST_FAMILY=0 -DOCT_INST_LOG2D=5|6|7|8     bit-packed kernel (sweep.cuh)
-//     -DOCT_INST_FAMILY=1 -DOCT_INST_LOG2D=5|6|7       link-entry kernel (sweep_links.cuh)
+//     -DOCT_INST_FAMILY=1 -DOCT_INST_LOG2D=5|6|7|8     link-entry kernel (sweep_links.cuh)
 // (paper_1705_01022_b200/build.py runs the compilations in parallel and links them with oct_api.cu).
 #include "launch.h"
 #include "sweep.cuh"
@@ -74,9 +74,11 @@ SweepLaunch make_links_launch(bool dead)
 #define OCT_LINK_SHAPES_A_5(X) X(5, 0, 0, 32, 4, 4) X(5, 1, 1, 16, 8, 4)
 #define OCT_LINK_SHAPES_A_6(X) X(6, 0, 0, 128, 1, 4) X(6, 1, 1, 32, 4, 4) X(6, 2, 1, 32, 4, 4) X(6, 2, 2, 16, 4, 2)
 #define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1, 4) X(7, 1, 1, 128, 1, 4) X(7, 2, 2, 64, 1, 2) X(7, 2, 1, 128, 1, 4) X(7, 3, 2, 32, 1, 2) X(7, 4, 1, 32, 1, 2)
+#define OCT_LINK_SHAPES_A_8(X) X(8, 1, 1, 512, 1, 2) X(8, 2, 1, 512, 1, 2) X(8, 2, 2, 256, 1, 2)
 #define OCT_LINK_SHAPES_B_5(X)
 #define OCT_LINK_SHAPES_B_6(X) X(6, 1, 1, 64, 2, 4) X(6, 2, 2, 16, 2, 4)
 #define OCT_LINK_SHAPES_B_7(X) X(7, 1, 1, 256, 1, 4) X(7, 2, 2, 64, 1, 4)
+#define OCT_LINK_SHAPES_B_8(X) X(8, 1, 1, 1024, 1, 2)
 
 bool OCT_CAT(oct_find_links_, OCT_INST_LOG2D)(int tx, int ty, int blk, bool variant_b, bool dead, SweepLaunch* out)
 {

@@ -67,7 +67,11 @@ struct LinkShape {
     static constexpr int BTW = (G_ == 16 && NSTEP > 64) ? 16 : (NSTEP < 64 ? NSTEP : 64);
     static constexpr int SMEM_PER_DOMAIN = (ENTRY_WORDS + BTW) * 4;
     static constexpr int SMEM_BYTES = SMEM_PER_DOMAIN * DPB;
-    static_assert(LOG2D <= 7, "x and y are decoded in 8-bit fields: D + CX - 2 must stay below 256");
+    // x and y of a site travel in one register: 8-bit fields (x | y << 8) while D + CX - 2 stays below 256, 16-bit fields
+    // (x | y << 16) for D = 256 -- two-byte entries only: a 256 x 256 window of four-byte entries does not fit shared memory
+    static constexpr bool WIDE = LOG2D == 8;
+    static constexpr int YSH = WIDE ? 16 : 8;
+    static_assert(LOG2D <= 7 || (LOG2D == 8 && EB == 2), "D = 256 needs two-byte entries");
     static_assert(NCELL % G == 0 && CPT >= 1, "every thread carries the same number of cells");
     static_assert(G == 16 || G % 32 == 0, "a group is half a warp or whole warps");
     // one warp or half a warp per 64 x 64 domain: the fast staging path (each window word is loaded once, the east
@@ -204,14 +208,26 @@ __device__ __forceinline__ uint32_t gather_word_rot(const uint32_t* __restrict__
     return word;
 }
 
-// entry index soff + y*P + x of the site packed as v = x | y << 8 (fields may hold x + D, y + D: cells wrap inside
-// the domain, R14): mask both fields at once, then one byte dot product (x, y, 0, 0) . (1, P, 0, 0) + soff
+// an (x | y << 8) pair with both fields below 256 in the register format of this shape
+template <class SH>
+__device__ __forceinline__ constexpr uint32_t widen(uint32_t f)
+{
+    return SH::WIDE ? ((f & 0xFFu) | ((f & 0xFF00u) << 8)) : f;
+}
+
+// entry index soff + y*P + x of the site packed as v = x | y << YSH (fields may hold x + D, y + D: cells wrap inside
+// the domain, R14): mask both fields at once, then one byte dot product (x, y, 0, 0) . (1, P, 0, 0) + soff (D = 256: the
+// pitch is no byte weight, shift and multiply-add)
 template <class SH>
 __device__ __forceinline__ uint32_t site_index(uint32_t v, uint32_t soff)
 {
-    static_assert(SH::P <= 255, "the pitch is a byte weight of the dot product");
-    const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
-    return __dp4a(vm, (uint32_t)(1 | (SH::P << 8)), soff);
+    const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << SH::YSH));
+    if constexpr (SH::WIDE) {
+        return (vm >> 16) * (uint32_t)SH::P + (vm & 0xFFFFu) + soff;
+    } else {
+        static_assert(SH::WIDE || SH::P <= 255, "the pitch is a byte weight of the dot product");
+        return __dp4a(vm, (uint32_t)(1 | (SH::P << 8)), soff);
+    }
 }
 
 // Carry out an accepted update at entry index `i` (relative to Sb): the site's four links flip.
@@ -300,7 +316,7 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
 #pragma unroll
     for (int j = 0; j < CPT; ++j) {
         const uint32_t c = tg + j * G;
-        cellc[j] = ((c & (SH::NCX - 1)) * CX) | (((c >> LOG2NCX) * CY) << 8);
+        cellc[j] = ((c & (SH::NCX - 1)) * CX) | (((c >> LOG2NCX) * CY) << SH::YSH);
     }
     const Rule<ONEDIR, ALWAYS, SH::EB> rule(P16, Q16);
 
@@ -308,8 +324,8 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
     auto decide_site = [&](uint32_t v, uint32_t w, uint32_t& idx) -> int {
         idx = site_index<SH>(v, soff);
         if constexpr (DEAD) {
-            const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
-            if ((vm & 0xFFu) >= dead_lim || (vm >> 8) >= dead_lim) return 0;      // dead border: not carried out
+            const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << SH::YSH));
+            if ((vm & (SH::WIDE ? 0xFFFFu : 0xFFu)) >= dead_lim || (vm >> SH::YSH) >= dead_lim) return 0;      // dead border: not carried out
         }
         if constexpr (SH::EB == 2) {
             const unsigned char* B2 = reinterpret_cast<const unsigned char*>(S) + 2u * idx;
@@ -336,10 +352,10 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
             if constexpr (BLK == kBlkDT)
-                o[kk] = ((((o[kk] >> 16) & 1u) * (CX / 2)) | ((((o[kk] >> 17) & 1u) * (CY / 2)) << 8))
-                        + (o[kk] & dtr_mask & (uint32_t)((CX - 1) | ((CY - 1) << 8)));
+                o[kk] = widen<SH>(((((o[kk] >> 16) & 1u) * (CX / 2)) | ((((o[kk] >> 17) & 1u) * (CY / 2)) << 8))
+                                  + (o[kk] & dtr_mask & (uint32_t)((CX - 1) | ((CY - 1) << 8))));
             else
-                o[kk] &= FM;
+                o[kk] = widen<SH>(o[kk] & FM);
         }
         *reinterpret_cast<uint4*>(BT + 4 * q) = make_uint4(o[0], o[1], o[2], o[3]);
     }
@@ -365,7 +381,7 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
-                    dec[j] = decide_site((w & FM) + cellc[j] + sc, w, idx[j]);
+                    dec[j] = decide_site(widen<SH>(w & FM) + cellc[j] + sc, w, idx[j]);
                 }
                 links_sync<G, SH::DPB>(grp, wmask);
 #pragma unroll
@@ -378,7 +394,7 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t f = rw[j][kk] & FM;
-                    vv[j] = f + cellc[j] + sc;
+                    vv[j] = widen<SH>(f) + cellc[j] + sc;
                     cls[j] = (uint32_t)((f & 0xFFu) == (uint32_t)(CX - 1)) + (uint32_t)((f >> 8) == (uint32_t)(CY - 1));
                 }
 #pragma unroll
@@ -399,7 +415,7 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) {
                     const uint32_t w = rw[j][kk];
-                    dec[j] = decide_site((w & FM) + cellc[j] + qc, w, idx[j]);
+                    dec[j] = decide_site(widen<SH>(w & FM) + cellc[j] + qc, w, idx[j]);
                 }
 #pragma unroll
                 for (int j = 0; j < CPT; ++j) rule.template apply<SH>(S, idx[j], dec[j], net);
