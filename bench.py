@@ -37,7 +37,7 @@ N_SM, SMSP, LANES = 148, 4, 32
 # (DESIGN.md section 5.1).  Four-byte entries: 1 entry load + 5 stores of an accepted update (issued whenever a lane of the
 # warp accepts); two-byte entries (shapes with few cells per domain): 3 loads + 3 stores.  Plus staging in and out,
 # 2 x ((D+4)^2 entries x EB bytes / 128 B) per D^2/32 warp-attempts of a domain, plus 1/8 block-step load.
-TWO_BYTE_SHAPES = {(6, 2, 2), (7, 2, 2), (7, 3, 2), (7, 4, 1)}          # (log2D, tcx, tcy), as built in csrc/sweep_inst.cu
+TWO_BYTE_SHAPES = {(6, 2, 2), (7, 2, 2), (7, 3, 2), (7, 4, 1), (8, 1, 1), (8, 2, 1), (8, 2, 2)}   # (log2D, tcx, tcy), as built in csrc/sweep_inst.cu
 
 
 def wavefronts_min(log2D: int, tcx: int, tcy: int, kernel_opt: int = 0) -> float:
@@ -319,7 +319,8 @@ def main():
     seed = replicas.replica_seed(args.seed, rank)
     warm = max(args.warmup, 3)
     peaks = measured_peaks()
-    kernel = "sweep_links_kernel" if (args.log2D <= 7 and args.kernel != 1) else "sweep_kernel"
+    links_shape = args.log2D <= 7 or (args.log2D == 8 and (args.tcx, args.tcy) in ((1, 1), (2, 1), (2, 2)))
+    kernel = "sweep_links_kernel" if (links_shape and args.kernel != 1) else "sweep_kernel"
 
     sim = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
     sim.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)
