@@ -76,7 +76,7 @@ SMALL = [
     (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 5, 1, 1, 2, 2), 0.9, 0.1, 8),
     (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DB, 6, 1, 1, 2, 3), 1.0, 0.0, 6),
     (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 7, 1, 1, 1, 1), 1.0, 0.0, 4),
-    (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8, 1, 1, 2, 1), 0.8, 0.2, 3),    # bit-packed kernel only (D = 256)
+    (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8, 1, 1, 2, 1), 0.8, 0.2, 3),    # D = 256: 16-bit coordinate fields, bit-wise write-back
     (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 2, 2, 1, 1), 1.0, 0.0, 6),    # two domains per warp
     (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 2, 1), 0.7, 0.3, 10),    # L = D, width 1: the tile is its own neighbour
     (64, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 5), 0.5, 0.5, 16),
