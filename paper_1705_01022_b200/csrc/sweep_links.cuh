@@ -251,6 +251,36 @@ __device__ __forceinline__ void flip_links(uint32_t* Sb, uint32_t i, bool up)
     B[+4 * SH::P + 2] = v0;         // north neighbour's S link = sigma_y(x,y+1)
 }
 
+// The same for a decision d in {-1, 0, +1} that differs from lane to lane in value AND direction (both rates non-zero):
+// written as predicated stores by hand -- left to the compiler, the `if (d != 0)` around stores whose values depend on d
+// becomes a divergent branch per cell and phase (BSSY / BRA / BSYNC; the mixed-rate sweep then ran 5x slower than p = 1).
+template <class SH>
+__device__ __forceinline__ void flip_links_signed(uint32_t* Sb, uint32_t i, int d)
+{
+    const bool up = d > 0;
+    if constexpr (SH::EB == 2) {
+        const uint32_t a = (uint32_t)__cvta_generic_to_shared(Sb) + 2u * i;
+        const uint32_t e = up ? 0xFFFFu : 0u, v0 = up ? 0u : 0xFFu;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %0, 0;\n\t"
+            "@p st.shared.u16 [%1], %2;\n\t"          // own W and S links
+            "@p st.shared.u8 [%1+2], %3;\n\t"         // east neighbour's W link
+            "@p st.shared.u8 [%1+%4], %3;\n\t}"       // north neighbour's S link
+            :: "r"(d), "r"(a), "r"(e), "r"(v0), "n"(2 * SH::P + 1) : "memory");
+    } else {
+        const uint32_t a = (uint32_t)__cvta_generic_to_shared(Sb + i);
+        const uint32_t e = up ? kEntryMax : kEntryMin, v1 = up ? 0xFFu : 0u, v0 = up ? 0u : 0xFFu;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %0, 0;\n\t"
+            "@p st.shared.u32 [%1], %2;\n\t"
+            "@p st.shared.u8 [%1+-3], %3;\n\t"        // west neighbour's E link
+            "@p st.shared.u8 [%1+4], %4;\n\t"         // east neighbour's W link
+            "@p st.shared.u8 [%1+%5], %3;\n\t"        // south neighbour's N link
+            "@p st.shared.u8 [%1+%6], %4;\n\t}"       // north neighbour's S link
+            :: "r"(d), "r"(a), "r"(e), "r"(v1), "r"(v0), "n"(-4 * SH::P + 3), "n"(4 * SH::P + 2) : "memory");
+    }
+}
+
 // Acceptance rule of one launch.  ONEDIR: only one of p, q is non-zero (always so for the sync variant),
 // so a single entry pattern is tested and the stored values are launch constants; ALWAYS: that live
 // threshold is 65536 (p = 1 or q = 1) and the 16-bit comparison is dropped as well.
@@ -269,8 +299,8 @@ struct Rule {
             if constexpr (!ALWAYS) acc = acc && (w >> 16) < T16;
             return acc ? (dep ? 1 : -1) : 0;
         } else {
-            const uint32_t r16 = w >> 16;
-            return (e == kMin && r16 < P16) ? 1 : ((e == kMax && r16 < Q16) ? -1 : 0);
+            const uint32_t r16 = w >> 16;                 // (no short-circuit operators: they compile to branches)
+            return (int)((e == kMin) & (r16 < P16)) - (int)((e == kMax) & (r16 < Q16));
         }
     }
     // carry out decision d at entry i and count it in net (deposits - removals; ONEDIR counts updates, the caller signs them)
@@ -278,7 +308,7 @@ struct Rule {
     __device__ __forceinline__ void apply(uint32_t* Sb, uint32_t i, int d, int& net) const
     {
         if constexpr (ONEDIR) { if (d != 0) { flip_links<SH>(Sb, i, dep); ++net; } }
-        else { if (d != 0) { flip_links<SH>(Sb, i, d > 0); net += d; } }
+        else { flip_links_signed<SH>(Sb, i, d); net += d; }
     }
 };
 
@@ -320,26 +350,34 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
     }
     const Rule<ONEDIR, ALWAYS, SH::EB> rule(P16, Q16);
 
-    // decision for the site packed in v (x | y << 8 before wrapping); idx receives its entry index
-    auto decide_site = [&](uint32_t v, uint32_t w, uint32_t& idx) -> int {
+    // decision for the site packed in v (x | y << YSH before wrapping); idx receives its entry index.  `live` = this cell
+    // takes part in the current phase (delayed borders): the loads are predicated, everything else is straight-line code, so
+    // a phase is no divergent branch.  An entry value of 0x55555555 is neither a minimum nor a maximum.
+    auto load_site = [&](uint32_t v, uint32_t& idx, bool live = true) -> uint32_t {
         idx = site_index<SH>(v, soff);
         if constexpr (DEAD) {
             const uint32_t vm = v & (uint32_t)((SH::D - 1) | ((SH::D - 1) << SH::YSH));
-            if ((vm & (SH::WIDE ? 0xFFFFu : 0xFFu)) >= dead_lim || (vm >> SH::YSH) >= dead_lim) return 0;      // dead border: not carried out
+            live = live && (vm & (SH::WIDE ? 0xFFFFu : 0xFFu)) < dead_lim && (vm >> SH::YSH) < dead_lim;      // dead border: not carried out
         }
+        uint32_t e = 0x55555555u;
         if constexpr (SH::EB == 2) {
             const unsigned char* B2 = reinterpret_cast<const unsigned char*>(S) + 2u * idx;
-            const uint32_t own = *reinterpret_cast<const unsigned short*>(B2), ea = B2[2], no = B2[2 * SH::P + 1];
-            return rule.decide(own | (ea << 16) | (no << 24), w);          // (W, S, E, N)
+            if (live) e = (uint32_t)*reinterpret_cast<const unsigned short*>(B2) | ((uint32_t)B2[2] << 16) | ((uint32_t)B2[2 * SH::P + 1] << 24);   // (W, S, E, N)
         } else {
-            return rule.decide(S[idx], w);
+            if (live) e = S[idx];
         }
+        return e;
     };
+    auto decide_site = [&](uint32_t v, uint32_t w, uint32_t& idx, bool live = true) -> int { return rule.decide(load_site(v, idx, live), w); };
     int net = 0;                                     // accepted updates of this lane's cells (counted under the stores' predicate)
 
     // a few groups of four steps per loop trip: the next groups' Philox rounds fill the issue slots the current
     // group's shared-memory round trips leave open (+3 % at D = 64, +8 % at D = 128 over no unrolling)
-    constexpr int kUnrollK4 = CPT >= 4 ? 2 : (SH::BTW / 4 < 8 / CPT ? SH::BTW / 4 : 8 / CPT);
+#ifndef OCT_DELAYED_UNROLL
+#define OCT_DELAYED_UNROLL 1
+#endif
+    // (delayed borders run three phases per step: one group of four steps per trip keeps the loop in the instruction cache)
+    constexpr int kUnrollK4 = BLK == kBlkDelayed ? OCT_DELAYED_UNROLL : CPT >= 4 ? 2 : (SH::BTW / 4 < 8 / CPT ? SH::BTW / 4 : 8 / CPT);
     constexpr uint32_t RB = SH::BTW / 4;             // groups of four steps per fill of the block-step ring
 #pragma unroll 1
     for (uint32_t kb = k4_begin; kb < k4_end; kb += RB) {
@@ -397,14 +435,58 @@ __device__ __forceinline__ int run_steps(uint32_t* __restrict__ S, uint32_t soff
                     vv[j] = widen<SH>(f) + cellc[j] + sc;
                     cls[j] = (uint32_t)((f & 0xFFu) == (uint32_t)(CX - 1)) + (uint32_t)((f >> 8) == (uint32_t)(CY - 1));
                 }
+                // The three phases only matter when two of the sites selected in this step are nearest neighbours (an update changes
+                // the four links of its site and nothing else, and a decision reads only the four links of its site): without such
+                // a pair every order gives the same lattice, and the step is ONE load-decide-store pass instead of three dependent
+                // ones.  A selected site's east (north) neighbour can only have been selected by the cell east (north) of it, so
+                // where a domain's cells sit in one warp two shuffles per cell slot find every pair; ~4 of 5 steps have none.
+                // The entries of all cells are loaded first (they are what the bulk phase, or the single pass, decides on), the
+                // shuffles run under the loads' latency.
+                uint32_t ent[CPT];
 #pragma unroll
-                for (uint32_t phase = 0; phase < 3; ++phase) {
-                    int dec[CPT];                    // cells of one phase never touch common links (R15): loads first
+                for (int j = 0; j < CPT; ++j) ent[j] = load_site(vv[j], idx[j]);
+                bool phased = true;
+                if constexpr (G <= 32 && SH::NCX <= G && !SH::WIDE) {
+                    constexpr uint32_t WRAP = (uint32_t)((SH::D - 1) | ((SH::D - 1) << 8));
+                    const uint32_t lane_base = (threadIdx.x & 31u) & ~(uint32_t)(G - 1);      // G = 16: the half warp of this domain
+                    bool pair = false;
 #pragma unroll
-                    for (int j = 0; j < CPT; ++j) dec[j] = cls[j] == phase ? decide_site(vv[j], rw[j][kk], idx[j]) : 0;
-    #pragma unroll
+                    for (int j = 0; j < CPT; ++j) {
+                        const uint32_t c = tg + j * G;
+                        const uint32_t ce = (c & ~(uint32_t)(SH::NCX - 1)) | ((c + 1u) & (uint32_t)(SH::NCX - 1));   // cell east of c (same slot)
+                        const uint32_t cn = (c + SH::NCX) & (uint32_t)(SH::NCELL - 1);                              // cell north of c
+                        const uint32_t me = vv[j] & WRAP;
+                        const uint32_t east = __shfl_sync(wmask, vv[j], lane_base | (ce & (uint32_t)(G - 1))) & WRAP;
+                        uint32_t north = 0u;
+#pragma unroll
+                        for (int jj = 0; jj < CPT; ++jj) {
+                            const uint32_t got = __shfl_sync(wmask, vv[jj], lane_base | (cn & (uint32_t)(G - 1)));
+                            if ((int)(cn / G) == jj) north = got & WRAP;
+                        }
+                        // (x = D - 1 or y = D - 1: me + 1 / me + 256 leaves the field, no wrapped coordinate equals it -- the halo is inactive)
+                        pair = pair || east == me + 1u || north == me + 256u;
+                    }
+                    phased = __any_sync(wmask, pair);
+                }
+                {
+                    // bulk phase, or (no nearest-neighbour pair) every cell: decisions on the entries loaded above
+                    int dec[CPT];
+#pragma unroll
+                    for (int j = 0; j < CPT; ++j) dec[j] = rule.decide((phased && cls[j] != 0u) ? 0x55555555u : ent[j], rw[j][kk]);
+#pragma unroll
                     for (int j = 0; j < CPT; ++j) rule.template apply<SH>(S, idx[j], dec[j], net);
                     links_sync<G, SH::DPB>(grp, wmask);
+                }
+                if (phased) {
+#pragma unroll
+                    for (uint32_t phase = 1; phase < 3; ++phase) {
+                        int dec[CPT];                    // cells of one phase never touch common links (R15): loads first
+#pragma unroll
+                        for (int j = 0; j < CPT; ++j) dec[j] = decide_site(vv[j], rw[j][kk], idx[j], cls[j] == phase);
+#pragma unroll
+                        for (int j = 0; j < CPT; ++j) rule.template apply<SH>(S, idx[j], dec[j], net);
+                        links_sync<G, SH::DPB>(grp, wmask);
+                    }
                 }
             } else {
                 // block-layer DT (:170): one random quadrant of every cell per step (R17).  The cells of a step
