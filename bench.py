@@ -286,6 +286,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="OCT_OPT_KERNEL value: 0 auto, 1 bit-packed, 2 link-entry variant B")
     ap.add_argument("--also-L", type=int, default=1 << 17, help="second lattice size measured in the same run (0: none)")
     ap.add_argument("--ensemble-L", type=int, default=1024, help="lattice edge of the ensemble (many lattices per launch) measurement (0: none)")
+    ap.add_argument("--no-shapes", dest="shapes", action="store_false", help="skip the other-shapes block")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-heights", action="store_true", help="skip timing oct_heights (needs a 4*L*L byte buffer)")
@@ -445,6 +446,25 @@ def main():
                 sm.close()
             del sims
 
+    # ---- other scheme shapes of the same workload (sweeps only, 8 MCS after 16 burn-in MCS): the paper's second production
+    # configuration TC=2,2 (Fig. 5 :236-244), larger domains, block-layer DT, and the mixed-rate path of BASELINE config 3 ------
+    shapes = None
+    if args.shapes and world == 1:
+        shapes = []
+        for log2D, tcx, tcy, blk, p_, q_ in ((6, 2, 2, 0, 1.0, 0.0), (7, 1, 1, 0, 1.0, 0.0), (8, 1, 1, 0, 1.0, 0.0), (6, 1, 1, 2, 1.0, 0.0),
+                                            (6, 1, 1, 0, 0.9, 0.1)):
+            code_s = wl.scheme_code(wl.DEV_DTR, blk, log2D, tcx, tcy)
+            sim_s = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
+            sim_s.oct_sweep(16, p_, q_, code_s)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); sim_s.oct_sweep(8, p_, q_, code_s); b.record(stream); torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            shapes.append({"scheme": wl.scheme_name(code_s), "p": p_, "q": q_, "L": L, "mcs": 8, "launch_ms": ms / 32,
+                           "attempts_per_s": 8 * L * L / (ms * 1e-3)})
+            sim_s.close()
+            del sim_s
+
     # ---- the oracle timed on this box's host cores (rank 0, N = 1 only): bounded samples ------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -465,7 +485,7 @@ def main():
                 "ms_per_step": m["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16 and args.blk == 0) else None,
                 "dtype": "u32", "data": "synthetic", "config": workload_config(args), "clocks": m["clocks"], "e2e": e2e,
-                "gpu_launches": m["launches"], "roofline": roofline, "sustained": sustained, "also": also, "ensemble": ensemble,
+                "gpu_launches": m["launches"], "roofline": roofline, "sustained": sustained, "also": also, "ensemble": ensemble, "shapes": shapes,
                 "observables": observables, "cpu_baseline": cpu,
                 "vs_cpu_baseline": (value / world / cpu["value"]) if cpu else None,
                 "paper_context": "vs_baseline divides by PAPER.md:276's ~9e9 attempts/s (DTrDB, L=2^16, p=1, q=0) on Kepler GPUs: other hardware, "
