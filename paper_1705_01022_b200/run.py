@@ -188,13 +188,15 @@ def main(argv=None):
     ap.add_argument("--tcy", type=int, default=1)
     ap.add_argument("--dev", type=int, default=wl.DEV_DTR)
     ap.add_argument("--blk", type=int, default=wl.BLK_DB)
+    ap.add_argument("--ka", type=int, default=0, help="dead-border layers: t_async = 2^-ka MCS (PAPER.md:204-206)")
+    ap.add_argument("--w", type=int, default=0, help="dead-border layers: border width in sites, 0 = the scheme's own (PAPER.md:202, :208)")
     ap.add_argument("--per-decade", type=int, default=8)
     ap.add_argument("--streams", type=int, default=0, help="ensemble: groups of members on concurrent CUDA streams (0: choose)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
 
     L, N = args.L, args.L * args.L
-    code = wl.scheme_code(args.dev, args.blk, args.log2D, args.tcx, args.tcy)
+    code = wl.scheme_code(args.dev, args.blk, args.log2D, args.tcx, args.tcy, args.ka, args.w)
     seeds = list(range(args.seed, args.seed + args.seeds))
     runs, wall = simulate(L, args.mcs, args.snap, args.p, args.q, code, seeds, args.per_decade, n_groups=args.streams)
     dt = binding.oct_time_per_sweep(L, code)
