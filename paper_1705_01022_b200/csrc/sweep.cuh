@@ -1,6 +1,7 @@
 // Sweep kernel, bit-packed window: one launch = one domain-set sweep of a DD scheme of arXiv 1705.01022
-// (Sec. 3).  This is the general kernel (every device layer incl. the dead-border schemes, D up to 256);
-// sweep_links.cuh holds the faster link-entry kernel that serves DTr/DT for D <= 128.
+// (Sec. 3).  This is the general kernel (every device layer incl. the dead-border schemes, every shape, D up to 256);
+// sweep_links.cuh holds the faster link-entry kernel, which serves every device layer for the shapes it is built for
+// (D <= 256) and is what AUTO picks there; this one remains the fallback and the second implementation of every parity case.
 //
 // B200 mapping (differs from the paper's Kepler kernel):
 //   * a device-layer domain (D x D sites) is owned by a small *worker group* of WPD
