@@ -42,7 +42,8 @@ extern "C" {
 
 typedef struct oct_ctx oct_ctx;   /* opaque host-side handle, owned by the library until oct_destroy */
 
-enum { OCT_OK = 0, OCT_EINVAL = -1, OCT_ECUDA = -2, OCT_ENOMEM = -3, OCT_ESTATE = -4 };
+enum { OCT_OK = 0, OCT_EINVAL = -1, OCT_ECUDA = -2, OCT_ENOMEM = -3, OCT_ESTATE = -4,
+       OCT_ETOOBIG = -5   /* oct_width2_static only: L is valid but beyond that call's fixed scratch */ };
 
 enum {
     OCT_INIT_FLAT = 0,          /* h = (x+y)&1: every word 0x33CC33CC, W^2 = 1/4 (R5)               */
@@ -126,6 +127,32 @@ int oct_heights(oct_ctx*, int32_t* heights_dev, void* stream);
  * c = h(0,0), S1 = sum (h-c), S2 = sum (h-c)^2 over all sites, net = deposits - removals so far.
  * Exact as long as L^2 * max (h-c)^2 < 2^63. */
 int oct_width2(oct_ctx*, int64_t* out_dev, void* stream);
+
+/* oct_width2 WITHOUT a handle and without a workspace: the same sums, out_dev[4] = {S1, S2, c, net} (Eq. (3) :61, R6),
+ * of the packed lattice at lattice_dev (canonical words, 16-byte aligned, L x L sites), with c = h00 and net passed
+ * in by value and copied through to out_dev[2], out_dev[3] (W^2 does not depend on c; pass 0, 0 if you do not track them).
+ *
+ * For callers that cannot allocate device memory at all, not even the workspace every other call needs: a measurement
+ * hook that is handed a lattice and a result slot by a program that owns all of HBM; code that must not call cudaMalloc /
+ * cudaFree because those synchronise the whole device and would stall the replicas sweeping on other streams; code in a
+ * part of the host program where allocation is forbidden or the memory budget is spent.  This call allocates nothing,
+ * on the device or through any library: its scratch (column 0 gathered, per-CTA net slopes, the L row anchors, two
+ * counters) is a fixed array inside the library image, 1024 + 5 * OCT_WIDTH2_STATIC_MAX_L = 328 704 bytes, which every
+ * GPU that loads the library holds until the process exits.
+ *
+ * LIMIT: 16 <= L <= OCT_WIDTH2_STATIC_MAX_L (2^16), a power of two.  A valid but larger L (2^17) returns OCT_ETOOBIG
+ * ("lattice larger than the fixed scratch of oct_width2_static"); nothing is enqueued and no memory is touched.
+ * FIRST CALL ON A DEVICE: looks up the device address of the array on the current device (cudaGetSymbolAddress, result
+ * checked, kept per device); make that first call with the right device current and before any stream capture begins.
+ * SHARED SCRATCH: all calls on one device use the same array, which keeps whatever the last call left.  That is
+ * harmless for calls that follow each other (each call writes every byte it later reads, and clears out_dev[0..3]
+ * itself), but two calls that can overlap on the GPU -- different streams, or different host threads without a common
+ * stream -- race on it and give garbage: put them on one stream or order them with events.
+ * Only ENQUEUES three launches on `stream`.  Results are the integers oct_width2 gives for the same lattice.
+ * Errors: EINVAL (null / misaligned pointer, L not a power of two or < 16), ETOOBIG, ECUDA (no sm_100 device, the symbol
+ * look-up or a launch failed). */
+#define OCT_WIDTH2_STATIC_MAX_L 65536u
+int oct_width2_static(const void* lattice_dev, uint32_t L, int64_t h00, int64_t net, int64_t* out_dev, void* stream);
 
 /* Waiting-time snapshot for aging (:75-80): copies the packed lattice to lattice_copy_dev
  * (oct_lattice_bytes, 16-byte aligned) and writes anchor_out_dev[2] = {h(0,0), net} at this moment. */

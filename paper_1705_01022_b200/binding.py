@@ -16,13 +16,15 @@ from . import build as _build
 from . import workloads as wl
 
 OCT_OK, OCT_EINVAL, OCT_ECUDA, OCT_ENOMEM, OCT_ESTATE = 0, -1, -2, -3, -4
+OCT_ETOOBIG = -5
+OCT_WIDTH2_STATIC_MAX_L = 1 << 16
 
 EXPORTS = (
     "oct_lattice_bytes", "oct_workspace_bytes", "oct_create", "oct_set_state", "oct_sweep", "oct_heights",
     "oct_width2", "oct_snapshot", "oct_autocorr", "oct_export", "oct_upload", "oct_counters", "oct_mcs",
     "oct_destroy", "oct_strerror", "oct_last_error", "oct_launch_count", "oct_w2_from_sums", "oct_c_from_sums",
     "oct_time_per_sweep", "oct_scheme_supported", "oct_set_option", "oct_slope_autocorr", "oct_cs_from_sums",
-    "oct_sweep_batch", "oct_observe", "oct_fetch", "oct_observe_batch",
+    "oct_sweep_batch", "oct_observe", "oct_fetch", "oct_observe_batch", "oct_width2_static",
 )
 OCT_OBS_W2, OCT_OBS_CH, OCT_OBS_CS = 1, 2, 4
 OCT_OPT_KERNEL = 1
@@ -71,6 +73,7 @@ def load(rebuild_if_stale: bool = True):
         "oct_slope_autocorr": (i32, [vp, vp, vp, vp]), "oct_cs_from_sums": (dbl, [u64, i64, i64, i64]),
         "oct_observe": (i32, [vp, i32, vp, vp, vp, vp]), "oct_fetch": (i32, [vp, vp, vp, sz, vp]),
         "oct_observe_batch": (i32, [C.POINTER(vp), u32, i32, C.POINTER(vp), C.POINTER(vp), vp, vp]),
+        "oct_width2_static": (i32, [vp, u32, i64, i64, vp, vp]),
     }
     for name in EXPORTS:
         fn = getattr(L, name)          # AttributeError if a declared symbol is not exported
@@ -142,6 +145,17 @@ def oct_observe_batch(sims, what: int, snapshots=None, anchors=None, out=None, s
     rc = load().oct_observe_batch(hs, n, what, sp, ap, out.data_ptr(), _stream_ptr(stream))
     if rc:
         raise OctError(rc, "oct_observe_batch", load().oct_last_error(sims[0]._h).decode() if sims else "")
+    return out
+
+
+def oct_width2_static(lattice, L: int, h00: int, net: int, out, stream=None):
+    """oct_width2's sums {S1, S2, c, net} of the packed lattice in the CUDA tensor `lattice`, written to the int64[4] CUDA
+    tensor `out` -- without a handle or workspace.  For callers that may not allocate device memory (see include/oct.h):
+    the C call allocates nothing, and neither does this wrapper, which is why `out` has no default.  L <= 2^16
+    (OctError with code OCT_ETOOBIG beyond); calls that can overlap on the GPU share one scratch array and race."""
+    rc = load().oct_width2_static(lattice.data_ptr(), L, h00, net, out.data_ptr(), _stream_ptr(stream))
+    if rc:
+        raise OctError(rc, "oct_width2_static")
     return out
 
 

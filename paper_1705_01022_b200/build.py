@@ -13,10 +13,10 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboct_b200.so")
 # translation units: (object name, source, extra defines).  sweep_inst.cu is compiled once per kernel family and
 # domain size so that the ~200 kernel instantiations build in parallel.
-UNITS = [("oct_api", "oct_api.cu", [])] + \
+UNITS = [("oct_api", "oct_api.cu", []), ("width2_static", "width2_static.cu", [])] + \
         [(f"packed_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=0", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7, 8)] + \
         [(f"links_{ld}", "sweep_inst.cu", ["-DOCT_INST_FAMILY=1", f"-DOCT_INST_LOG2D={ld}"]) for ld in (5, 6, 7, 8)]
-HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "observe_rows.cuh", "philox.cuh", "launch.h", "sweep_inst.cu", "oct_api.cu",
+HEADERS = ["sweep.cuh", "sweep_links.cuh", "observe.cuh", "observe_rows.cuh", "philox.cuh", "launch.h", "sweep_inst.cu", "oct_api.cu", "width2_static.cu",
            os.path.join("..", "..", "include", "oct.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "--use_fast_math", "-Xptxas", "-v"]
@@ -41,6 +41,7 @@ def stale() -> bool:
 # what each translation unit includes: a unit is recompiled when one of these (or this file) is newer than its object
 UNIT_DEPS = {"oct_api.cu": ["oct_api.cu", "observe.cuh", "observe_rows.cuh", "philox.cuh", "launch.h", "sweep.cuh",
                             os.path.join("..", "..", "include", "oct.h")],
+             "width2_static.cu": ["width2_static.cu", "observe.cuh", "observe_rows.cuh", os.path.join("..", "..", "include", "oct.h")],
              "sweep_inst.cu": ["sweep_inst.cu", "launch.h", "sweep.cuh", "sweep_links.cuh", "philox.cuh"]}
 
 

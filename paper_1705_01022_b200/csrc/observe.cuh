@@ -92,6 +92,9 @@ __device__ __forceinline__ void column_anchor_body(const uint32_t* __restrict__ 
     }
 }
 
+// A second translation unit that only wants the device bodies and parameter blocks of this header (width2_static.cu)
+// defines OCT_OBSERVE_BODIES_ONLY: the non-template kernels below have external linkage and must exist once per library.
+#ifndef OCT_OBSERVE_BODIES_ONLY
 // the lattices k = blockIdx.y (one or two: current lattice and snapshot)
 __global__ void __launch_bounds__(kColThreads)
 column_gather_kernel(const uint32_t* __restrict__ lat0, const uint32_t* __restrict__ lat1, uint32_t L,
@@ -107,6 +110,8 @@ column_anchor_kernel(const uint32_t* __restrict__ col0, const uint32_t* __restri
     column_anchor_body(blockIdx.y ? col1 : col0, blocksum + blockIdx.y * kColMaxBlocks, L, blockIdx.y ? anchor1 : anchor0, zero,
                        blockIdx.y ? 0 : n_zero);
 }
+
+#endif  // OCT_OBSERVE_BODIES_ONLY
 
 // ---- kernel 2 -------------------------------------------------------------------------------------
 
@@ -142,6 +147,7 @@ struct ObsBatchParams {
     ObsMember m[kMaxObsBatch];
 };
 
+#ifndef OCT_OBSERVE_BODIES_ONLY
 __global__ void __launch_bounds__(kColThreads) column_gather_batch_kernel(const __grid_constant__ ObsBatchParams BP)
 {
     const ObsMember& mb = BP.m[blockIdx.z];
@@ -209,5 +215,7 @@ __global__ void set_counters_kernel(unsigned long long* counters, long long h00,
     counters[0] = (unsigned long long)net;
     counters[1] = (unsigned long long)h00;
 }
+
+#endif  // OCT_OBSERVE_BODIES_ONLY
 
 }  // namespace octb

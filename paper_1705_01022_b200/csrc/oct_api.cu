@@ -643,6 +643,7 @@ const char* oct_strerror(int code)
         case OCT_ECUDA: return "CUDA error (see oct_last_error)";
         case OCT_ENOMEM: return "out of host memory";
         case OCT_ESTATE: return "invalid state";
+        case OCT_ETOOBIG: return "lattice larger than the fixed scratch of oct_width2_static (L <= 65536)";
         default: return "unknown error code";
     }
 }
