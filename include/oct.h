@@ -16,6 +16,8 @@
  *  - ONE STREAM PER HANDLE at a time: the observables share scratch in the handle's workspace (the column
  *    anchors), so calls on one handle must be ordered (same stream, or the caller's events).  Different
  *    handles are independent and may run on different streams concurrently.
+ *  - One process may drive several GPUs: a handle belongs to the device that was current at oct_create (its buffers
+ *    live there); make that device current again for every call on the handle.  Nothing is cached across devices.
  *  - The library runs on the current CUDA device and requires compute capability 10.x; there is no
  *    CPU fallback: without a usable device every compute call returns OCT_ECUDA.
  *  - Determinism: the lattice after oct_sweep depends only on (L, seed, init, the sequence of
@@ -114,9 +116,12 @@ int oct_sweep(oct_ctx*, uint64_t n_mcs, double p, double q, int scheme, void* st
  * oct_sweep on that handle alone would give.  The two halves of the ensemble run side by side -- one on `stream`, one on
  * a helper stream of handle 0 that forks from `stream` and joins it again before the call returns -- so that the last
  * domains of one half's launch overlap the other half's next launch; for the caller everything is ordered on `stream`.
- * Shapes without a many-lattices kernel (D = 128 other than TC=1,1, the bit-packed kernel) run the members one after the
- * other.  The kernel option of handle 0 applies.
- * Errors: as oct_sweep, plus EINVAL for n = 0, a null or repeated handle, or members of different L. */
+ * Shapes without a many-lattices kernel (D = 128 other than TC=1,1, every D = 256 shape, the bit-packed kernel) run the
+ * members one after the other.  The kernel option of handle 0 applies.
+ * Errors: as oct_sweep, plus EINVAL for n = 0, a null or repeated handle, or members of different L.  A CUDA failure
+ * between two MCS returns ECUDA with every member's clock at the sweeps completed (as oct_sweep).  A failure INSIDE an
+ * MCS -- some launches of its domain sets enqueued, others not -- returns ESTATE: the members' lattices then hold a partly
+ * swept MCS that no clock value describes; re-create or re-upload them (oct_last_error(handles[0]) has the CUDA text). */
 int oct_sweep_batch(oct_ctx* const* handles, uint32_t n, uint64_t n_mcs, double p, double q, int scheme, void* stream);
 
 /* Integrate the slopes into int32 heights h[y*L+x] (:52 "peaks of the octahedra define the height

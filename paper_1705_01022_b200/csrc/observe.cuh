@@ -124,6 +124,7 @@ struct RowsParams {
     const long long* snapB;                 // {h00, net} of the snapshot
     int32_t* heights;                       // heights_kernel output
     unsigned long long* out;                // rows3_kernel: [0..3] W^2 sums, [4..8] C_h sums, [9..14] C_s sums
+    unsigned long long* out_ch;             // where the five C_h sums go: out + 4 in the 16-slot layout, the caller's buffer itself for oct_autocorr
     uint32_t L;
 };
 

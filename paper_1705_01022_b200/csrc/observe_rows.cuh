@@ -233,13 +233,13 @@ __device__ __forceinline__ void rows3_body(const RowsParams& P)
             atomicAdd(&P.out[1], (unsigned long long)t2);
         }
         if constexpr (CH) {
-            atomicAdd(&P.out[4], (unsigned long long)t1);
-            atomicAdd(&P.out[5], (unsigned long long)t3);
-            atomicAdd(&P.out[6], (unsigned long long)t4);
+            atomicAdd(&P.out_ch[0], (unsigned long long)t1);
+            atomicAdd(&P.out_ch[1], (unsigned long long)t3);
+            atomicAdd(&P.out_ch[2], (unsigned long long)t4);
         }
         if (blockIdx.x == 0) {
             if constexpr (W2) { P.out[2] = P.countersA[1]; P.out[3] = P.countersA[0]; }                         // c = h(0,0), net
-            if constexpr (CH) { P.out[7] = P.countersA[1]; P.out[8] = (unsigned long long)P.snapB[0]; }         // c_t, c_s
+            if constexpr (CH) { P.out_ch[3] = P.countersA[1]; P.out_ch[4] = (unsigned long long)P.snapB[0]; }         // c_t, c_s
         }
     }
     if constexpr (CS) {
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(kRows2Warps * 32) rows3_batch_kernel(const __g
     const ObsMember& mb = BP.m[blockIdx.y];
     RowsParams P;
     P.latA = mb.latA; P.latB = mb.latB; P.anchorA = mb.anchorA; P.anchorB = mb.anchorB; P.countersA = mb.countersA;
-    P.snapB = mb.snapB; P.heights = nullptr; P.out = mb.out; P.L = BP.L;
+    P.snapB = mb.snapB; P.heights = nullptr; P.out = mb.out; P.out_ch = mb.out + 4; P.L = BP.L;
     rows3_body<WHAT, RUN>(P);
 }
 

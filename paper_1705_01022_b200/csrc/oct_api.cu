@@ -281,8 +281,8 @@ int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
     pl->P16 = prob16(p); pl->Q16 = prob16(q);
     const int blk = (f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR) ? kBlkDT
                   : (f.blk == OCT_BLK_DB_DELAYED || (pl->P16 > 0 && pl->Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
-    // the link-entry kernel serves domains that fit shared memory unpacked; the bit-packed kernel serves
-    // everything else (D = 256, domains with fewer than 16 cells)
+    // the link-entry kernel serves every (D, TC) it is instantiated for (sweep_inst.cu: D <= 128, and D = 256 with
+    // TC=1,1 / 2,1 / 2,2 as two-byte entries); the bit-packed kernel serves the rest (TC=3,1 / 1,3 at D = 64, TC=3,2 / 4,1 at D = 256)
     const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED &&
                        find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B,
                                          f.dev > OCT_DEV_DT, &pl->sl);
@@ -296,15 +296,15 @@ int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
     return OCT_OK;
 }
 
-// kernels that need more than 48 KiB of dynamic shared memory are opted in once per function
+// Kernels that need more than 48 KiB of dynamic shared memory must be opted in.  The attribute belongs to the function ON
+// THE CURRENT DEVICE, so a process that drives several GPUs has to set it on each of them; remembering "done" per function
+// pointer (as this code once did) leaves the second device without it and every large launch there fails.  Setting it
+// costs a few microseconds next to the 4 * n_mcs launches of the call, so it is simply set on every sweep call: no cache,
+// nothing shared between host threads.
 int opt_in_smem(oct_ctx* c, const void* fn, int smem)
 {
-    static const void* done[64];
-    static int n_done = 0;
     if (smem <= 48 * 1024) return OCT_OK;
-    for (int i = 0; i < n_done; ++i) if (done[i] == fn) return OCT_OK;
     OCT_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    if (n_done < 64) done[n_done++] = fn;
     return OCT_OK;
 }
 
@@ -393,9 +393,19 @@ int oct_sweep_batch(oct_ctx* const* cs, uint32_t n, uint64_t n_mcs, double p, do
     const uint32_t n_half = n >= 2 ? (n + 1) / 2 : n;
     const bool two = n >= 2;
     if (two && !c0->aux) {
-        OCT_CUDA(c0, cudaStreamCreateWithFlags(&c0->aux, cudaStreamNonBlocking));
-        OCT_CUDA(c0, cudaEventCreateWithFlags(&c0->ev_fork, cudaEventDisableTiming));
-        OCT_CUDA(c0, cudaEventCreateWithFlags(&c0->ev_join, cudaEventDisableTiming));
+        // all three or none: a handle with a helper stream but no events would fail on every later batch call
+        cudaStream_t aux = nullptr;
+        cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+        cudaError_t e = cudaStreamCreateWithFlags(&aux, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming);
+        if (e != cudaSuccess) {
+            if (ev_join) cudaEventDestroy(ev_join);
+            if (ev_fork) cudaEventDestroy(ev_fork);
+            if (aux) cudaStreamDestroy(aux);
+            return fail_cuda(c0, e, "oct_sweep_batch: helper stream / events");
+        }
+        c0->aux = aux; c0->ev_fork = ev_fork; c0->ev_join = ev_join;
     }
     if (two) {
         OCT_CUDA(c0, cudaEventRecord(c0->ev_fork, st));
@@ -403,9 +413,11 @@ int oct_sweep_batch(oct_ctx* const* cs, uint32_t n, uint64_t n_mcs, double p, do
     }
     SweepBatchParams bp{};
     fill_common(bp.common, c0, pl);
-    int rc_launch = OCT_OK;
-    for (uint64_t i = 0; i < n_mcs && rc_launch == OCT_OK; ++i) {
-        for (uint32_t half = 0; half < (two ? 2u : 1u) && rc_launch == OCT_OK; ++half) {
+    cudaError_t e_launch = cudaSuccess;      // the first failure, kept: cudaGetLastError() hands an error out only once
+    bool partial = false;                    // a failure after part of an MCS was enqueued
+    for (uint64_t i = 0; i < n_mcs && e_launch == cudaSuccess; ++i) {
+        uint32_t enq = 0;
+        for (uint32_t half = 0; half < (two ? 2u : 1u) && e_launch == cudaSuccess; ++half) {
             const uint32_t h0 = half ? n_half : 0u, h1 = half ? n : n_half;
             cudaStream_t hs = half ? c0->aux : st;
             for (uint32_t m0 = h0; m0 < h1; m0 += kMaxBatch) {       // at most kMaxBatch members per launch
@@ -414,22 +426,30 @@ int oct_sweep_batch(oct_ctx* const* cs, uint32_t n, uint64_t n_mcs, double p, do
                     const oct_ctx* c = cs[m0 + m];
                     bp.m[m] = BatchMember{c->lat, c->counters(), (uint32_t)c->seed, (uint32_t)(c->seed >> 32), (uint32_t)c->t, 0u};
                 }
-                for (uint32_t si = 0; si < pl.n_launch; ++si) {
+                for (uint32_t si = 0; si < pl.n_launch && e_launch == cudaSuccess; ++si) {
                     bp.common.si = si;
-                    if (launch_sweep(pl.sl.kern_batch, dim3(pl.grid, nb), pl.sl.threads, pl.sl.smem, hs, bp, pl.pdl) != cudaSuccess) rc_launch = OCT_ECUDA;
-                    c0->launches++;
+                    e_launch = launch_sweep(pl.sl.kern_batch, dim3(pl.grid, nb), pl.sl.threads, pl.sl.smem, hs, bp, pl.pdl);
+                    if (e_launch == cudaSuccess) { c0->launches++; ++enq; }
                 }
             }
         }
-        if (rc_launch == OCT_OK && cudaGetLastError() != cudaSuccess) rc_launch = OCT_ECUDA;
-        if (rc_launch == OCT_OK)
+        if (e_launch == cudaSuccess) e_launch = cudaGetLastError();
+        if (e_launch == cudaSuccess)
             for (uint32_t m = 0; m < n; ++m) cs[m]->t++;
+        else if (enq) partial = true;
     }
     if (two) {                                                       // join, whatever happened: the caller's stream stays the only one to wait on
         cudaEventRecord(c0->ev_join, c0->aux);
         cudaStreamWaitEvent(st, c0->ev_join, 0);
     }
-    if (rc_launch != OCT_OK) return fail_cuda(c0, cudaGetLastError(), "oct_sweep_batch launch");
+    if (e_launch != cudaSuccess) {
+        (void)cudaGetLastError();                                    // leave no stale error for the caller's next CUDA call
+        // Some members may have received 1..3 of the 4 domain sets of the failing MCS while no clock was advanced for it:
+        // their lattices are no longer a function of (seed, t).  Say so instead of pretending the state is resumable.
+        const int rc_fail = fail_cuda(c0, e_launch, partial ? "oct_sweep_batch launch (members hold a partly enqueued MCS: re-create or re-upload them)"
+                                                            : "oct_sweep_batch launch");
+        return partial ? OCT_ESTATE : rc_fail;
+    }
     return OCT_OK;
 }
 
@@ -485,7 +505,7 @@ int oct_autocorr(oct_ctx* c, const void* snapshot_dev, const int64_t* snapshot_a
     rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
     rp.anchorA = c->anchorA(); rp.anchorB = c->anchorB(); rp.countersA = c->counters();
     rp.snapB = reinterpret_cast<const long long*>(snapshot_anchor_dev);
-    rp.out = reinterpret_cast<unsigned long long*>(out_dev) - 4; rp.L = c->L;      // the kernel writes slots 4..8
+    rp.out = nullptr; rp.out_ch = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;   // C_h sums only: the kernel touches out_ch[0..4]
     const uint32_t LW = c->L >> 2;
     launch_rows(kObsCh, rp, LW, st);
     c->launches++;
@@ -523,7 +543,7 @@ int oct_observe(oct_ctx* c, int what, const void* snapshot_dev, const int64_t* s
     rp.latA = c->lat; rp.latB = static_cast<const uint32_t*>(snapshot_dev);
     rp.anchorA = c->anchorA(); rp.anchorB = c->anchorB(); rp.countersA = c->counters();
     rp.snapB = reinterpret_cast<const long long*>(snapshot_anchor_dev);
-    rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.L = c->L;
+    rp.out = reinterpret_cast<unsigned long long*>(out_dev); rp.out_ch = rp.out + 4; rp.L = c->L;
     launch_rows(what, rp, c->L >> 2, st);
     c->launches++;
     OCT_CUDA(c, cudaGetLastError());

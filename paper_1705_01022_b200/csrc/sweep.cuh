@@ -64,7 +64,10 @@ __device__ __forceinline__ uint32_t tile_bits(uint32_t iw, uint32_t jw, uint32_t
 }
 
 // write back one window word of a dead-border tile: whole if it holds only this tile's sites (or the border is wide
-// enough that foreign bits cannot change, dead_w >= 4), else only this tile's bits
+// enough that foreign bits cannot change, dead_w >= 4), else only this tile's bits.  The neighbouring tile stages the
+// same word in with a plain load while this one may be writing it: harmless, because a tile consumes only ITS OWN bits
+// of a shared word (the foreign bits belong to dead sites: never tested, never written back), and those bits are
+// written by nobody else during the launch.
 __device__ __forceinline__ void store_tile_word(uint32_t* ptr, uint32_t word, uint32_t iw, uint32_t jw, uint32_t offx, uint32_t offy,
                                                 uint32_t D, uint32_t dead_w)
 {
@@ -233,9 +236,15 @@ sweep_kernel(const __grid_constant__ SweepParams P)
     const bool has00 = x00 < (uint32_t)D && y00 < (uint32_t)D;
 
     // ---- a2: stage-in (:164) ---------------------------------------------------------------------
+    // Dead-border layers: window words past the last column / row that holds one of this tile's active sites (or their
+    // E / N links) belong to the next tile, which writes them in this same launch.  They are neither tested nor written
+    // back here, so they are not loaded either (zeros stand in), as kept() does in sweep_links.cuh: no cross-CTA
+    // read of a word another CTA is writing.
+    const uint32_t ncol = dead ? ((offx + (uint32_t)D - dead_w) >> 2) + 1u : (uint32_t)NW;
+    const uint32_t nrow = dead ? ((offy + (uint32_t)D - dead_w) >> 2) + 1u : (uint32_t)NW;
     for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
         const uint32_t j = idx / NW, i = idx - j * NW;
-        S[j * PITCH + i] = P.lat[(size_t)((wy0 + j) & LWm) * LW + ((wx0 + i) & LWm)];
+        S[j * PITCH + i] = (i < ncol && j < nrow) ? P.lat[(size_t)((wy0 + j) & LWm) * LW + ((wx0 + i) & LWm)] : 0u;
     }
     // ---- a3: block-step table (:170, :172; R13/R17/R24) ------------------------------------------
     const uint32_t c2b = (kTagBlock << 30) | (set << 28) | dom, c2c = (kTagCell << 30) | (set << 28) | dom;
@@ -340,7 +349,6 @@ sweep_kernel(const __grid_constant__ SweepParams P)
 
     // ---- a7: stage-out (:164).  Whole words; for dead-border schemes the words that also hold the
     // next tile's sites are never modified here and are not written (:166) ------------------------
-    const uint32_t ncol = ((offx + (uint32_t)D - dead_w) >> 2) + 1u, nrow = ((offy + (uint32_t)D - dead_w) >> 2) + 1u;
     for (uint32_t idx = tg; idx < (uint32_t)(NW * NW); idx += G) {
         const uint32_t j = idx / NW, i = idx - j * NW;
         if (i < ncol && j < nrow) {

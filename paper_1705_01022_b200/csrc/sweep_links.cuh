@@ -1,6 +1,7 @@
 // Sweep kernel, link-entry layout: one launch = one domain-set sweep of any device-layer scheme of
 // arXiv 1705.01022 (DTr / DT: Sec. 3.0.2-3.0.3; DB / cDB / DBh: Sec. 3.0.1, :133-140, :166)
-// with any of the single-hit block layers (Sec. 3.1, :168-174), for device-layer domains of D <= 128 sites.
+// with any of the single-hit block layers (Sec. 3.1, :168-174), for device-layer domains of D <= 256 sites (D = 256 with
+// two-byte entries only: four-byte entries of a 256 x 256 domain do not fit shared memory).
 //
 // Why a second layout (profiles/r1_a_*.md): on the bit-packed window the update test costs ~115 SASS
 // instructions per attempt, almost all of them shift/mask arithmetic and shared-memory atomics, and the

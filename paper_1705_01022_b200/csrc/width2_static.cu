@@ -85,7 +85,7 @@ width2_static_rows_kernel(const uint32_t* __restrict__ lat, uint32_t L, const un
     P.latA = lat; P.latB = nullptr;
     P.anchorA = reinterpret_cast<const int32_t*>(scratch + kOffAnchor); P.anchorB = nullptr;
     P.countersA = reinterpret_cast<const unsigned long long*>(scratch + kOffCounters);
-    P.snapB = nullptr; P.heights = nullptr; P.out = out; P.L = L;
+    P.snapB = nullptr; P.heights = nullptr; P.out = out; P.out_ch = nullptr; P.L = L;
     rows3_body<kObsW2, RUN>(P);
 }
 
