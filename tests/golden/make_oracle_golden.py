@@ -34,6 +34,10 @@ RUNS = (
     ("cDBDT_D64", 256, 2, 1.0, 0.0, scheme(DEV_CDB, BLK_DT, 6), (5,)),
     ("DBhDB_D64", 256, 2, 0.8, 0.2, scheme(DEV_DBH, BLK_DB, 6), (5,)),
     ("DTrDB_TC22_D128", 256, 4, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 7, 2, 2), (4,)),
+    # seeds that use the HIGH half of the 64-bit Philox key (R19: key = (seed & 2^32-1, seed >> 32)); every run above has it zero
+    ("DTrDB_delayed_seed64", 256, 0x9E3779B97F4A7C15, 0.9, 0.1, scheme(DEV_DTR, BLK_DB, 6), (6,)),
+    ("DBDB_TC22_seedhi7", 256, (7 << 32) | 1, 1.0, 0.0, scheme(DEV_DB, BLK_DB, 6, 2, 2), (4,)),
+    ("DTrDB_seedhi_only", 256, 1 << 32, 1.0, 0.0, scheme(DEV_DTR, BLK_DB, 6), (3,)),
 )
 
 
@@ -49,6 +53,9 @@ FULL_RUNS = {
     # BASELINE config 3: L = 4096, p = 0.9, q = 0.1, seed 7, DTrDB (delayed borders), the whole 5000-MCS run:
     # lattice hash every 500 MCS, and the sums after EVERY MCS hashed per 500-MCS window
     "c3_D128": (4096, 7, 0.9, 0.1, scheme(DEV_DTR, BLK_DB, 7), tuple(range(500, 5001, 500)), True),
+    # the same run with D = 64, the shape whose domains sit in one warp: there the CUDA path decides per collective step
+    # whether the delayed-border phases can be merged into one pass
+    "c3_D64": (4096, 7, 0.9, 0.1, scheme(DEV_DTR, BLK_DB, 6), tuple(range(500, 5001, 500)), True),
 }
 
 

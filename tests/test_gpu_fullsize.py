@@ -93,11 +93,16 @@ def check_invariants(sim, words):
     return S1, S2, c, net
 
 
-@pytest.mark.parametrize("log2D,kernel", [(6, binding.OCT_KERNEL_AUTO), (7, binding.OCT_KERNEL_AUTO), (8, binding.OCT_KERNEL_AUTO)])
-def test_config3_L65536_sampled_boxes(log2D, kernel):
-    """BASELINE config 4: L = 2^16, p = 1, q = 0, flat start, seed 1, DTrDB TC=1,1."""
-    L, seed, p, q = 1 << 16, 1, 1.0, 0.0
-    code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, log2D)
+@pytest.mark.parametrize("log2D,tc,p,q", [(6, 1, 1.0, 0.0), (7, 1, 1.0, 0.0), (8, 1, 1.0, 0.0),
+                                          (6, 1, 0.9, 0.1),      # mixed rates at D = 64: the one-pass / three-phase decision per step
+                                          (6, 2, 1.0, 0.0),      # TC=2,2: two-byte entries, two domains per warp
+                                          (6, 2, 0.9, 0.1)],
+                         ids=["D64", "D128", "D256", "D64-mixed", "D64-TC22", "D64-TC22-mixed"])
+def test_config3_L65536_sampled_boxes(log2D, tc, p, q):
+    """BASELINE config 4: L = 2^16, flat start, seed 1, DTrDB -- TC=1,1 with p = 1, q = 0 as the config states it, and the
+    other shapes bench.py times at this size (`shapes`: mixed rates, TC=2,2), at the MCS it times them (24 -> 25)."""
+    L, seed, kernel = 1 << 16, 1, binding.OCT_KERNEL_AUTO
+    code = wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, log2D, tc, tc)
     sim = binding.Sim(L, seed)
     sim.oct_set_option(binding.OCT_OPT_KERNEL, kernel)
     # the very first MCS, from the flat state (acceptance 1/2)
@@ -119,6 +124,7 @@ def test_config3_L65536_sampled_boxes(log2D, kernel):
     S1, S2, c, net = check_invariants(sim, post)
     assert net > 0 and S2 > 0
     sim.close()
+    del pre, post
 
 
 def test_config4_L131072_sampled_boxes():

@@ -95,7 +95,7 @@ SMALL = [
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 3, 2), 1.0, 0.0, 3),         # Fig. 4 cell shapes at D = 128
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 7, 4, 1), 1.0, 0.0, 3),
     (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 4, 1), 0.8, 0.2, 2),
-    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 1.0, 0.0, 6),               # D = 256: 4 warps, named CTA barrier
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 1.0, 0.0, 6),               # D = 256: one 512-thread CTA per domain, two-byte entries, __syncthreads
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 0.9, 0.1, 4),
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 8), 1.0, 0.0, 4),
     (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8), 1.0, 0.0, 4),
@@ -119,6 +119,76 @@ def test_sweep_bit_exact(L, code, p, q, n):
         sim = gpu_run(L, seed, code, n, p, q, kernel=k)
         compare_state(sim, orc, check_heights=(name == "auto"))
         sim.close()
+    orc.close()
+
+
+SEEDS64 = (0x9E3779B97F4A7C15, (7 << 32) | 1, 1 << 32)
+
+
+@pytest.mark.parametrize("seed", SEEDS64, ids=[hex(s) for s in SEEDS64])
+def test_seeds_with_a_high_half_reach_every_kernel_family(seed):
+    """The Philox key is the 64-bit seed as (low word, high word) (R19).  Every other case in this file has a seed
+    below 2^32, i.e. a zero second key word: here the high half is live in each kernel family -- four-byte link
+    entries, two-byte entries (TC=2,2 at D = 64, D = 256), the alternative work split, the bit-packed kernel, a
+    dead-border layer, delayed borders, the DT block layer."""
+    cases = [(256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 1.0, 0.0, 4),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 0.9, 0.1, 4),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 3),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 7), 0.7, 0.3, 3),
+             (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 1, 1, 1), 1.0, 0.0, 3),
+             (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8), 1.0, 0.0, 2)]
+    for L, code, p, q, n in cases:
+        orc = Oracle(L, seed)
+        orc.sweep(n, p, q, code)
+        low = Oracle(L, seed & 0xFFFFFFFF)
+        low.sweep(n, p, q, code)
+        assert (low.lattice != orc.lattice).any(), "the high half of the seed does not reach the oracle's streams"
+        low.close()
+        for name, k in KERNELS.items():
+            sim = gpu_run(L, seed, code, n, p, q, kernel=k)
+            compare_state(sim, orc, check_heights=False)
+            sim.close()
+        orc.close()
+
+
+def test_batch_members_that_differ_only_in_the_high_half_of_the_seed():
+    """oct_sweep_batch builds each member's round keys in registers from (seed_lo, seed_hi): members with one low word
+    and different high words must each follow their own oracle run."""
+    L, n = 256, 3
+    for code, p, q in ((wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6), 1.0, 0.0), (wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 0.8, 0.2),
+                       (wl.scheme_code(wl.DEV_DB, wl.BLK_DT, 6), 0.6, 0.4), (wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 1.0, 0.0)):
+        seeds = [5, (1 << 32) | 5, (0xDEADBEEF << 32) | 5, (1 << 63) | 5]
+        sims = [binding.Sim(L, sd) for sd in seeds]
+        binding.oct_sweep_batch(sims, n, p, q, code)
+        words = []
+        for sim, sd in zip(sims, seeds):
+            orc = Oracle(L, sd)
+            orc.sweep(n, p, q, code)
+            compare_state(sim, orc, check_heights=False)
+            words.append(orc.lattice.copy())
+            orc.close()
+            sim.close()
+        for i in range(len(words)):
+            for j in range(i):
+                assert (words[i] != words[j]).any()
+
+
+def test_a_second_device_in_the_same_process():
+    """One process may drive several GPUs (replicas are this path's only multi-GPU mode): the > 48 KiB shared-memory
+    opt-in is per device, so a shape that needs it (D = 128: 70 KiB) must also launch on the second device used."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    L, code, n = 256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 3
+    orc = Oracle(L, 21)
+    orc.sweep(n, 1.0, 0.0, code)
+    try:
+        for dev in ("cuda:0", "cuda:1", "cuda:0"):
+            sim = binding.Sim(L, 21, device=dev)          # makes `dev` current
+            sim.oct_sweep(n, 1.0, 0.0, code)
+            compare_state(sim, orc, check_heights=False)
+            sim.close()
+    finally:
+        torch.cuda.set_device(0)
     orc.close()
 
 
