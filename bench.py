@@ -48,6 +48,40 @@ def wavefronts_min(log2D: int, tcx: int, tcy: int, kernel_opt: int = 0) -> float
 
 
 WAVEFRONTS_MIN = wavefronts_min(6, 1, 1)
+
+
+def expected_max_bank_load(n_lanes, n_banks=32, trials=20000, seed=12345):
+    """E[max number of lanes that fall into one bank] for n_lanes accesses at independent uniformly random banks: the
+    wavefronts one shared-memory instruction costs when its lanes address unrelated 32-bit words.
+    n_lanes may be an array of per-trial lane counts (stores: only the accepting lanes are live)."""
+    import numpy as np
+    rng = np.random.default_rng(seed)
+    n = np.broadcast_to(np.asarray(n_lanes), (trials,))
+    banks = rng.integers(0, n_banks, size=(trials, 32))
+    live = np.arange(32)[None, :] < n[:, None]
+    occ = np.zeros((trials, n_banks), dtype=np.int64)
+    np.add.at(occ, (np.repeat(np.arange(trials), 32)[live.ravel()], banks.ravel()[live.ravel()]), 1)
+    return float(occ.max(axis=1).mean())
+
+
+def wavefronts_expected_linear(log2D, tcx, tcy, kernel_opt, acceptance, trials=20000):
+    """Expected shared-memory wavefronts per warp-attempt of the link-entry sweep in ANY layout that is linear in the site
+    coordinates (entry address = y * pitch + x): the 32 lanes of a collective step address 32 unrelated sites, so every
+    load costs E[max bank load of 32 random banks] ~ 3.5 wavefronts instead of 1, and every store instruction -- issued
+    for the warp whenever a lane accepts, with only the accepting lanes live -- E[max(1, max bank load of n)] with
+    n ~ Binomial(32, acceptance).  Staging and the block-step load stay conflict-free.  This is the ceiling of the layout,
+    not of the hardware: roofline.frac is quoted against the conflict-free minimum, frac_of_layout_ceiling against this."""
+    import numpy as np
+    eb = 2 if ((log2D, tcx, tcy) in TWO_BYTE_SHAPES and kernel_opt != 2) else 4
+    n_loads, n_stores = (1, 5) if eb == 4 else (3, 3)
+    rng = np.random.default_rng(777)
+    load = expected_max_bank_load(32, trials=trials)
+    n_acc = rng.binomial(32, acceptance, size=trials)
+    store = expected_max_bank_load(np.maximum(n_acc, 1), trials=trials)
+    conflict_free_rest = wavefronts_min(log2D, tcx, tcy, kernel_opt) - 6.0
+    return {"wavefronts_expected_linear": n_loads * load + n_stores * store + conflict_free_rest, "per_load": load, "per_store": store,
+            "acceptance": acceptance, "loads": n_loads, "stores": n_stores,
+            "model": "lanes at independent uniformly random banks (32 banks x 4 B); stores with Binomial(32, acceptance) live lanes"}
 # Algorithmic lane-instructions per attempt (DESIGN.md section 7): Philox 40/4 = 10, site select 5, entry load +
 # compare 2, five stores + accept count 6, loop/sync 1, staging per site 6 (permute expansion 47/16, gather 34/16, loads,
 # stores and addresses).  The executed count comes from the committed ncu capture.
@@ -63,7 +97,7 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
 
 
-def ncu_counters(kernel: str, L: int, log2D: int, tcx: int, tcy: int, blk: int):
+def ncu_counters(kernel: str, L: int, log2D: int, tcx: int, tcy: int, blk: int, p: float = 1.0, q: float = 0.0):
     """Per-launch counters of the sweep kernel from the committed ncu capture (profiles/sweep_counters.csv: one row per
     captured configuration; the .md beside it names the command).  None if this configuration was not captured."""
     path = os.path.join(ROOT, "profiles", "sweep_counters.csv")
@@ -73,7 +107,8 @@ def ncu_counters(kernel: str, L: int, log2D: int, tcx: int, tcy: int, blk: int):
     hdr = rows[0]
     for r in rows[1:]:
         d = dict(zip(hdr, r))
-        if (d["kernel"], int(d["L"]), int(d["log2D"]), int(d["tcx"]), int(d["tcy"]), int(d["blk"])) == (kernel, L, log2D, tcx, tcy, blk):
+        if (d["kernel"], int(d["L"]), int(d["log2D"]), int(d["tcx"]), int(d["tcy"]), int(d["blk"]), float(d.get("p", 1.0)), float(d.get("q", 0.0))) == \
+                (kernel, L, log2D, tcx, tcy, blk, float(p), float(q)):
             return {k: (float(v) if k not in ("kernel", "source") else v) for k, v in d.items()}
     return None
 
@@ -139,8 +174,11 @@ def baseline_config_no(L):
 def workload_config(args, oracle_sample_L=None):
     n = baseline_config_no(args.L)
     tag = f"BASELINE config {n}" if n else "custom size"
-    cfg = {"workload": f"{tag}: octahedron model, L={args.L} periodic, flat start, p=1 q=0, {scheme_label(args)}",
-           "L": args.L, "p": 1.0, "q": 0.0, "scheme": scheme_label(args), "mcs_per_step": args.mcs_per_step,
+    pp, qq = getattr(args, "p", 1.0), getattr(args, "q", 0.0)
+    if (pp, qq) != (1.0, 0.0):
+        tag = "custom rates"
+    cfg = {"workload": f"{tag}: octahedron model, L={args.L} periodic, flat start, p={pp:g} q={qq:g}, {scheme_label(args)}",
+           "L": args.L, "p": pp, "q": qq, "scheme": scheme_label(args), "mcs_per_step": args.mcs_per_step,
            "burn_in_mcs": args.burn_in, "l2": "inputs larger than L2 (lattice %d MiB)" % (args.L * args.L // 4 >> 20),
            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
     if oracle_sample_L is not None:
@@ -190,7 +228,7 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line), flush=True)
 
 
-def measure(sim, code, M, steps, warmup, torch, dist, replicas, binding, snap, anchor, obs_out, sampler=None):
+def measure(sim, code, M, steps, warmup, torch, dist, replicas, binding, snap, anchor, obs_out, sampler=None, p=1.0, q=0.0):
     """warmup + `steps` timed steps of (M MCS of oct_sweep, then W^2 and C_h sums in one pass); CUDA events on the stream."""
     stream = torch.cuda.current_stream()
     what = binding.OCT_OBS_W2 | binding.OCT_OBS_CH
@@ -198,7 +236,7 @@ def measure(sim, code, M, steps, warmup, torch, dist, replicas, binding, snap, a
     def step(ev=None):
         if ev:
             ev[0].record(stream)
-        sim.oct_sweep(M, 1.0, 0.0, code)
+        sim.oct_sweep(M, p, q, code)
         if ev:
             ev[1].record(stream)
         sim.oct_observe(what, snap, anchor, obs_out)
@@ -231,7 +269,7 @@ def measure(sim, code, M, steps, warmup, torch, dist, replicas, binding, snap, a
             "window_ms": per_step_sweep}
 
 
-def roofline_block(args, L, peaks, sweep_ms, total_ms, n_sweep_launches, kernel):
+def roofline_block(args, L, peaks, sweep_ms, total_ms, n_sweep_launches, kernel, acceptance=None):
     """Roofline of the dominant kernel (one domain-set sweep): shared-memory data pipe, with the issue-slot view beside it."""
     launch_s = sweep_ms * 1e-3 / n_sweep_launches
     attempts_per_launch = L * L / 4
@@ -240,7 +278,8 @@ def roofline_block(args, L, peaks, sweep_ms, total_ms, n_sweep_launches, kernel)
     peak_wf = N_SM * f_hz / 1e9                                    # G wavefronts/s: one per clock per SM
     wf_min = wavefronts_min(args.log2D, args.tcx, args.tcy, args.kernel)
     achieved = wf_min * warp_attempts / launch_s / 1e9
-    cnt = ncu_counters(kernel, L, args.log2D, args.tcx, args.tcy, args.blk) or ncu_counters(kernel, 1 << 16, args.log2D, args.tcx, args.tcy, args.blk)
+    pq = (getattr(args, "p", 1.0), getattr(args, "q", 0.0))
+    cnt = ncu_counters(kernel, L, args.log2D, args.tcx, args.tcy, args.blk, *pq) or ncu_counters(kernel, 1 << 16, args.log2D, args.tcx, args.tcy, args.blk, *pq)
     rf = {"bound": "smem", "achieved": achieved, "peak": peak_wf, "unit": "Gwavefront/s", "frac": achieved / peak_wf,
           "traffic": None, "kernel": kernel, "avg_launch_ms": launch_s * 1e3, "attempts_per_launch": attempts_per_launch,
           "wavefronts_per_warp_attempt_min": wf_min,
@@ -263,6 +302,10 @@ def roofline_block(args, L, peaks, sweep_ms, total_ms, n_sweep_launches, kernel)
         issue["frac_executed"] = issue["achieved_executed"] / peak_issue
         rf["counters_src"] = cnt["source"]
     rf["issue_slots"] = issue
+    if acceptance is not None and kernel == "sweep_links_kernel":
+        lc = wavefronts_expected_linear(args.log2D, args.tcx, args.tcy, args.kernel, acceptance)
+        lc["frac_of_layout_ceiling"] = lc["wavefronts_expected_linear"] * warp_attempts / launch_s / 1e9 / peak_wf
+        rf["layout_ceiling"] = lc
     return rf
 
 
@@ -277,6 +320,8 @@ def main():
     ap.add_argument("--mcs-per-step", type=int, default=32)
     ap.add_argument("--burn-in", type=int, default=32)
     ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--p", type=float, default=1.0, help="deposition probability of the timed workload (BASELINE config 4: 1)")
+    ap.add_argument("--q", type=float, default=0.0, help="removal probability (config 4: 0; config 3's mixed rates: --p 0.9 --q 0.1)")
     ap.add_argument("--ref-L", type=int, default=4096, help="lattice edge of the oracle's timed sample")
     ap.add_argument("--ref-mcs", type=int, default=16)
     ap.add_argument("--ref-burn", type=int, default=4)
@@ -287,6 +332,8 @@ def main():
     ap.add_argument("--also-L", type=int, default=1 << 17, help="second lattice size measured in the same run (0: none)")
     ap.add_argument("--ensemble-L", type=int, default=1024, help="lattice edge of the ensemble (many lattices per launch) measurement (0: none)")
     ap.add_argument("--no-shapes", dest="shapes", action="store_false", help="skip the other-shapes block")
+    ap.add_argument("--sustained-windows", type=int, default=3, help="windows of the sustained-throughput protocol (0: skip)")
+    ap.add_argument("--sustained-window-mcs", type=int, default=100, help="MCS per window (at least 100)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-heights", action="store_true", help="skip timing oct_heights (needs a 4*L*L byte buffer)")
@@ -326,11 +373,17 @@ def main():
     sim = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
     sim.oct_set_option(binding.OCT_OPT_KERNEL, args.kernel)
     stream = torch.cuda.current_stream()
-    sim.oct_sweep(args.burn_in, 1.0, 0.0, code)            # evolved state: acceptance ~0.2 (not the flat 0.5)
+    sim.oct_sweep(args.burn_in, args.p, args.q, code)      # evolved state: acceptance ~0.2 (not the flat 0.5)
     snap, anchor = sim.oct_snapshot()
     obs = torch.empty(16, dtype=torch.int64, device=sim.device)
+    net_before = sim.oct_counters()[1]
     m = measure(sim, code, M, args.steps, warm, torch, dist, replicas, binding, snap, anchor, obs,
-                sampler=ClockSampler(local_rank) if rank == 0 else None)
+                sampler=ClockSampler(local_rank) if rank == 0 else None, p=args.p, q=args.q)
+    # acceptance over warm-up + timed steps: with one rate zero every accepted update moves the net counter by one
+    # (mixed rates: deposits and removals cancel in it, so no figure and no layout ceiling there)
+    acceptance = None
+    if args.p == 0.0 or args.q == 0.0:
+        acceptance = abs(sim.oct_counters()[1] - net_before) / float((warm + args.steps) * M * L * L)
     barrier = m["barrier"]
     attempts_per_step = M * L * L
     value = replicas.aggregate_throughput(attempts_per_step, args.steps, world, m["total_ms"])
@@ -340,10 +393,35 @@ def main():
     h00, net = sim.oct_counters()
     assert S[2] == h00 and S[3] == net and S[0] + L * L * h00 == L * L // 2 + 2 * net and S[4] == S[0], "inconsistent state"
 
-    roofline = roofline_block(args, L, peaks, m["sweep_ms"], m["total_ms"], args.steps * M * 4, kernel)
-    # sustained throughput: the sweep part of every timed step is a window of M MCS (PAPER.md:268 saw clocks drop after ~100 MCS)
-    win = sorted(L * L * M / (w * 1e-3) for w in m["window_ms"])
-    sustained = {"window_mcs": M, "windows": len(win), "median_attempts_per_s": win[len(win) // 2], "min": win[0], "max": win[-1]}
+    roofline = roofline_block(args, L, peaks, m["sweep_ms"], m["total_ms"], args.steps * M * 4, kernel, acceptance)
+    # Sustained throughput, the protocol of SURVEY 8(d): the paper saw its GPU clock down after ~100 MCS (PAPER.md:262, :268,
+    # Fig. 7), so the figure is the MEDIAN over windows of >= 100 MCS that start after >= 200 MCS of load.  Everything
+    # above (burn-in, warm-up, the timed steps) is that load; the windows are sweeps only, timed with CUDA events, with the
+    # clock sampler running.
+    sustained = None
+    if args.sustained_windows > 0:
+        mcs_before = args.burn_in + (warm + args.steps) * M
+        extra = max(0, 200 - mcs_before)
+        if extra:
+            sim.oct_sweep(extra, args.p, args.q, code)
+        Wm = max(100, args.sustained_window_mcs)
+        smp = ClockSampler(local_rank) if rank == 0 else None
+        evw = [torch.cuda.Event(enable_timing=True) for _ in range(args.sustained_windows + 1)]
+        barrier()
+        if smp is not None:
+            smp.start()
+        evw[0].record(stream)
+        for i in range(args.sustained_windows):
+            sim.oct_sweep(Wm, args.p, args.q, code)
+            evw[i + 1].record(stream)
+        barrier()
+        wclk = smp.stop() if smp is not None else None
+        wms = [evw[i].elapsed_time(evw[i + 1]) for i in range(args.sustained_windows)]
+        wms = replicas.max_over_ranks(wms, dist, sim.device)
+        win = sorted(world * L * L * Wm / (w * 1e-3) for w in wms)
+        sustained = {"window_mcs": Wm, "windows": len(win), "mcs_of_load_before_first_window": mcs_before + extra,
+                     "median_attempts_per_s": statistics.median(win), "min": win[0], "max": win[-1], "clocks": wclk,
+                     "protocol": "median over windows of >= 100 MCS after >= 200 MCS of load (SURVEY 8(d); PAPER.md:262, :268)"}
 
     # ---- observables (a8/a9): HBM-bound kernels, timed alone, algorithmic bytes / time -------------------
     def time_call(fn, reps=5):
@@ -385,7 +463,7 @@ def main():
 
         def step_e2e():
             sim.oct_upload(host.data_ptr())                          # the lattice exported by the previous step: counters stay valid
-            sim.oct_sweep(M, 1.0, 0.0, code)
+            sim.oct_sweep(M, args.p, args.q, code)
             sim.oct_observe(binding.OCT_OBS_W2 | binding.OCT_OBS_CH, snap, anchor, obs)
             sim.oct_fetch(obs, sums_host.data_ptr(), 16 * 8)         # synchronises
             sim.oct_export_to(host.data_ptr())                       # synchronises
@@ -483,13 +561,16 @@ def main():
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
                 "ms_per_step": m["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16 and args.blk == 0) else None,
+                "vs_baseline": None,
                 "dtype": "u32", "data": "synthetic", "config": workload_config(args), "clocks": m["clocks"], "e2e": e2e,
                 "gpu_launches": m["launches"], "roofline": roofline, "sustained": sustained, "also": also, "ensemble": ensemble, "shapes": shapes,
                 "observables": observables, "cpu_baseline": cpu,
                 "vs_cpu_baseline": (value / world / cpu["value"]) if cpu else None,
-                "paper_context": "vs_baseline divides by PAPER.md:276's ~9e9 attempts/s (DTrDB, L=2^16, p=1, q=0) on Kepler GPUs: other hardware, "
-                                 "context, not a target; vs_cpu_baseline divides by the oracle timed in this run (cpu_baseline.sample says on what)"}
+                "paper_context": {"paper_attempts_per_s": PAPER_ATTEMPTS_PER_S,
+                                  "value_over_paper": (value / world / PAPER_ATTEMPTS_PER_S) if (L == 1 << 16 and args.blk == 0 and args.p == 1.0 and args.q == 0.0) else None,
+                                  "note": "PAPER.md:276: ~9e9 attempts/s for DTrDB at L=2^16, p=1, q=0 on Kepler GPUs -- another machine's number: context, "
+                                          "not a baseline (vs_baseline stays null; BASELINE.json publishes none); vs_cpu_baseline divides by the oracle "
+                                          "timed in this run (cpu_baseline.sample says on what)"}}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -3,7 +3,7 @@
 // with any of the single-hit block layers (Sec. 3.1, :168-174), for device-layer domains of D <= 256 sites (D = 256 with
 // two-byte entries only: four-byte entries of a 256 x 256 domain do not fit shared memory).
 //
-// Why a second layout (profiles/r1_a_*.md): on the bit-packed window the update test costs ~115 SASS
+// Why a second layout (profiles/r3_sweep.md, last section): on the bit-packed window the update test costs ~115 SASS
 // instructions per attempt, almost all of them shift/mask arithmetic and shared-memory atomics, and the
 // ALU pipe binds.  Here the window is unpacked ONCE per domain sweep into one 32-bit *entry* per site that
 // carries the four links of that site, one byte each (0x00 = slope -1, 0xFF = slope +1):
