@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import shutil
 import subprocess
@@ -30,8 +31,18 @@ def nvcc() -> str:
     return exe
 
 
+STAMP = LIB + ".flags"      # hash of the flags the library on disk was built with (absent: the default flags)
+
+
+def _flags_hash(extra_flags=()) -> str:
+    return hashlib.sha256(" ".join([*NVCC_FLAGS, *extra_flags]).encode()).hexdigest()[:12]
+
+
 def stale() -> bool:
+    """True if the library is missing, older than a source, or was linked from an experiment build (extra_flags)."""
     if not os.path.exists(LIB):
+        return True
+    if os.path.exists(STAMP) and open(STAMP).read().strip() != _flags_hash():
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in HEADERS] + [os.path.abspath(__file__)]
@@ -54,19 +65,23 @@ def _unit_stale(obj: str, src: str, force: bool) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False, ptxas_info: str | None = None, extra_flags=()) -> str:
-    """Compile the stale units (in parallel; all of them with force=True or extra_flags), link liboct_b200.so.  Objects are
-    kept under build/ (git-ignored) so that a change to one header recompiles only the units that include it.
+    """Compile the stale units (in parallel; all of them with force=True), link liboct_b200.so.  Objects are kept under
+    build/<flags hash>/ (git-ignored) so that a change to one header recompiles only the units that include it, and a build
+    with extra_flags (always linked, even when the default library is up to date) never shares objects with the default one.
     ptxas_info: optional path that receives ptxas' per-kernel register / spill / shared-memory report of the units that
     were compiled; extra_flags: additional nvcc flags (e.g. -D switches)."""
-    if not (force or stale()):
+    if not (force or extra_flags or stale()):
         return LIB
-    os.makedirs(OBJDIR, exist_ok=True)
+    # objects live under build/<hash of every flag that shapes them>: an experiment build (extra_flags) can never leave
+    # objects behind that a later default build would take for its own
+    objdir = os.path.join(OBJDIR, _flags_hash(extra_flags))
+    os.makedirs(objdir, exist_ok=True)
     tag = f".tmp{os.getpid()}"
     procs, objs = [], []
     for name, src, defs in UNITS:
-        obj = os.path.join(OBJDIR, name + ".o")
+        obj = os.path.join(objdir, name + ".o")
         objs.append(obj)
-        if _unit_stale(obj, src, force or bool(extra_flags)):
+        if _unit_stale(obj, src, force):
             cmd = [nvcc(), *NVCC_FLAGS, *defs, *extra_flags, "-c", "-o", obj + tag, os.path.join(CSRC, src)]
             procs.append((name, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
     report, failed = [], None
@@ -93,6 +108,8 @@ def build(force: bool = False, verbose: bool = False, ptxas_info: str | None = N
         with open(ptxas_info, "w") as f:
             f.write("".join(l for e in report for l in e.splitlines(True) if "Compile time" not in l))
     os.replace(tmp, LIB)
+    with open(STAMP, "w") as f:
+        f.write(_flags_hash(extra_flags) + "\n")
     return LIB
 
 
