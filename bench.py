@@ -332,6 +332,7 @@ def main():
     ap.add_argument("--also-L", type=int, default=1 << 17, help="second lattice size measured in the same run (0: none)")
     ap.add_argument("--ensemble-L", type=int, default=1024, help="lattice edge of the ensemble (many lattices per launch) measurement (0: none)")
     ap.add_argument("--no-shapes", dest="shapes", action="store_false", help="skip the other-shapes block")
+    ap.add_argument("--shapes-all", action="store_true", help="the other-shapes block over every Fig. 4 cell shape x D x kernel option x rate set (minutes)")
     ap.add_argument("--sustained-windows", type=int, default=3, help="windows of the sustained-throughput protocol (0: skip)")
     ap.add_argument("--sustained-window-mcs", type=int, default=100, help="MCS per window (at least 100)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -529,16 +530,22 @@ def main():
     shapes = None
     if args.shapes and world == 1:
         shapes = []
-        for log2D, tcx, tcy, blk, p_, q_ in ((6, 2, 2, 0, 1.0, 0.0), (7, 1, 1, 0, 1.0, 0.0), (8, 1, 1, 0, 1.0, 0.0), (6, 1, 1, 2, 1.0, 0.0),
-                                            (6, 1, 1, 0, 0.9, 0.1)):
+        shape_list = [(6, 2, 2, 0, 1.0, 0.0, 0), (6, 3, 1, 0, 1.0, 0.0, 0), (7, 1, 1, 0, 1.0, 0.0, 0), (8, 1, 1, 0, 1.0, 0.0, 0), (6, 1, 1, 2, 1.0, 0.0, 0),
+                      (6, 1, 1, 0, 0.9, 0.1, 0), (7, 1, 1, 0, 0.9, 0.1, 0)]
+        if args.shapes_all:      # every cell shape of the Fig. 4 caption at every D it is built for, both kernels, both rate sets
+            shape_list = [(ld, tx, ty, 0, p_, q_, k_) for ld, tx, ty in ((6, 1, 1), (6, 2, 1), (6, 2, 2), (6, 3, 1), (6, 1, 3), (7, 1, 1), (7, 2, 2), (7, 3, 1),
+                                                                          (7, 1, 3), (7, 3, 2), (7, 4, 1), (8, 1, 1), (8, 2, 2), (8, 3, 2), (8, 4, 1))
+                          for p_, q_ in ((1.0, 0.0), (0.9, 0.1)) for k_ in (0, 1)]
+        for log2D, tcx, tcy, blk, p_, q_, k_ in shape_list:
             code_s = wl.scheme_code(wl.DEV_DTR, blk, log2D, tcx, tcy)
             sim_s = binding.Sim(L, seed, wl.INIT_FLAT, device=f"cuda:{local_rank}")
+            sim_s.oct_set_option(binding.OCT_OPT_KERNEL, k_)
             sim_s.oct_sweep(16, p_, q_, code_s)
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream); sim_s.oct_sweep(8, p_, q_, code_s); b.record(stream); torch.cuda.synchronize()
             ms = a.elapsed_time(b)
-            shapes.append({"scheme": wl.scheme_name(code_s), "p": p_, "q": q_, "L": L, "mcs": 8, "launch_ms": ms / 32,
+            shapes.append({"scheme": wl.scheme_name(code_s), "p": p_, "q": q_, "kernel_option": k_, "L": L, "mcs": 8, "launch_ms": ms / 32,
                            "attempts_per_s": 8 * L * L / (ms * 1e-3)})
             sim_s.close()
             del sim_s

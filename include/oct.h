@@ -214,7 +214,7 @@ const char* oct_last_error(const oct_ctx*);             /* text of the last CUDA
 
 /* Implementation options.  They never change results (every kernel is bit-identical to the oracle), only
  * which kernel runs.  OCT_OPT_KERNEL: AUTO picks the link-entry kernel (one entry of four or two link bytes per site
- * in shared memory, no atomics) wherever one is built (D <= 128; D = 256 with TC=1,1, 2,1, 2,2) and the bit-packed
+ * in shared memory, no atomics) wherever one is built (every accepted (D, TC) except D = 32 with TC=2,2) and the bit-packed
  * kernel otherwise; BITPACKED forces the latter; LINKS_B selects the alternative work split (another number of
  * warps per domain) or entry size (four link bytes per site instead of two, for TC=2,2) where one is built.
  * EINVAL for unknown options / values. */

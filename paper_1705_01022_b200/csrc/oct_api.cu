@@ -281,9 +281,12 @@ int plan_sweep(oct_ctx* c, double p, double q, int scheme, SweepPlan* pl)
     pl->P16 = prob16(p); pl->Q16 = prob16(q);
     const int blk = (f.blk == OCT_BLK_DT || f.blk == OCT_BLK_DTR) ? kBlkDT
                   : (f.blk == OCT_BLK_DB_DELAYED || (pl->P16 > 0 && pl->Q16 > 0)) ? kBlkDelayed : kBlkSync;   // R16
-    // the link-entry kernel serves every (D, TC) it is instantiated for (sweep_inst.cu: D <= 128, and D = 256 with
-    // TC=1,1 / 2,1 / 2,2 as two-byte entries); the bit-packed kernel serves the rest (TC=3,1 / 1,3 at D = 64, TC=3,2 / 4,1 at D = 256)
-    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED &&
+    // the link-entry kernel serves every (D, TC) it is instantiated for (sweep_inst.cu: every shape the library accepts
+    // except D = 32 TC=2,2, D = 256 as two-byte entries); the bit-packed kernel serves the rest and kernel option 1
+    // one measured exception (profiles/r3_shapes.md): delayed borders at D = 256 with 128 cells per domain (TC=3,2 / 4,1) run
+    // 11 % faster on the bit-packed kernel (one 128-thread CTA per SM cannot hide three CTA barriers per step)
+    const bool packed_wins = f.log2D == 8 && f.tcx + f.tcy >= 5 && blk == kBlkDelayed && c->opt_kernel == OCT_KERNEL_AUTO;
+    const bool links = c->opt_kernel != OCT_KERNEL_BITPACKED && !packed_wins &&
                        find_links_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, c->opt_kernel == OCT_KERNEL_LINKS_B,
                                          f.dev > OCT_DEV_DT, &pl->sl);
     if (!links && !find_launch((int)f.log2D, (int)f.tcx, (int)f.tcy, blk, &pl->sl)) return OCT_EINVAL;

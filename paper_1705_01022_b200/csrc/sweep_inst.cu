@@ -32,7 +32,7 @@ SweepLaunch make_launch()
 
 #define OCT_SHAPES_5(X) X(5, 0, 0) X(5, 1, 1) X(5, 2, 2)
 #define OCT_SHAPES_6(X) X(6, 0, 0) X(6, 1, 1) X(6, 2, 2) X(6, 2, 1) X(6, 3, 1) X(6, 1, 3)
-#define OCT_SHAPES_7(X) X(7, 0, 0) X(7, 1, 1) X(7, 2, 2) X(7, 2, 1) X(7, 3, 2) X(7, 4, 1)
+#define OCT_SHAPES_7(X) X(7, 0, 0) X(7, 1, 1) X(7, 2, 2) X(7, 2, 1) X(7, 3, 2) X(7, 4, 1) X(7, 3, 1) X(7, 1, 3)
 #define OCT_SHAPES_8(X) X(8, 1, 1) X(8, 2, 2) X(8, 2, 1) X(8, 3, 2) X(8, 4, 1)
 
 bool OCT_CAT(oct_find_packed_, OCT_INST_LOG2D)(int tx, int ty, int blk, SweepLaunch* out)
@@ -72,9 +72,9 @@ SweepLaunch make_links_launch(bool dead)
 }
 
 #define OCT_LINK_SHAPES_A_5(X) X(5, 0, 0, 32, 4, 4) X(5, 1, 1, 16, 8, 4)
-#define OCT_LINK_SHAPES_A_6(X) X(6, 0, 0, 128, 1, 4) X(6, 1, 1, 32, 4, 4) X(6, 2, 1, 32, 4, 4) X(6, 2, 2, 16, 4, 2)
-#define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1, 4) X(7, 1, 1, 128, 1, 4) X(7, 2, 2, 64, 1, 2) X(7, 2, 1, 128, 1, 4) X(7, 3, 2, 32, 1, 2) X(7, 4, 1, 32, 1, 2)
-#define OCT_LINK_SHAPES_A_8(X) X(8, 1, 1, 512, 1, 2) X(8, 2, 1, 512, 1, 2) X(8, 2, 2, 256, 1, 2)
+#define OCT_LINK_SHAPES_A_6(X) X(6, 0, 0, 128, 1, 4) X(6, 1, 1, 32, 4, 4) X(6, 2, 1, 32, 4, 4) X(6, 2, 2, 16, 4, 2) X(6, 3, 1, 16, 4, 2) X(6, 1, 3, 16, 4, 2)
+#define OCT_LINK_SHAPES_A_7(X) X(7, 0, 0, 256, 1, 4) X(7, 1, 1, 128, 1, 4) X(7, 2, 2, 64, 1, 2) X(7, 2, 1, 128, 1, 4) X(7, 3, 2, 32, 1, 2) X(7, 4, 1, 32, 1, 2) X(7, 3, 1, 64, 1, 2) X(7, 1, 3, 64, 1, 2)
+#define OCT_LINK_SHAPES_A_8(X) X(8, 1, 1, 512, 1, 2) X(8, 2, 1, 512, 1, 2) X(8, 2, 2, 256, 1, 2) X(8, 3, 2, 128, 1, 2) X(8, 4, 1, 128, 1, 2)
 #define OCT_LINK_SHAPES_B_5(X)
 #define OCT_LINK_SHAPES_B_6(X) X(6, 1, 1, 64, 2, 4) X(6, 2, 2, 16, 2, 4)
 #define OCT_LINK_SHAPES_B_7(X) X(7, 1, 1, 256, 1, 4) X(7, 2, 2, 64, 1, 4)

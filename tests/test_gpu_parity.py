@@ -102,6 +102,22 @@ SMALL = [
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8, 2, 2), 1.0, 0.0, 4),
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8, 3, 2), 0.9, 0.1, 4),
     (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 8, 4, 1), 1.0, 0.0, 4),
+    # the remaining cell shapes of the Fig. 4 caption on the link-entry kernel: TC=3,1 / 1,3 at D = 64 (16 cells:
+    # half-warp groups) and D = 128 (64 cells), TC=3,2 / 4,1 at D = 256 (128 cells); every block layer, dead borders too
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 3, 1), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB_DELAYED, 6, 1, 3), 1.0, 0.0, 4),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 1, 3), 0.9, 0.1, 5),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 6, 3, 1), 0.7, 0.3, 4),
+    (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6, 1, 3, 1, 1), 1.0, 0.0, 6),
+    (256, wl.scheme_code(wl.DEV_CDB, wl.BLK_DT, 6, 3, 1), 0.6, 0.4, 4),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 3, 1), 1.0, 0.0, 4),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7, 1, 3), 0.8, 0.2, 3),
+    (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 7, 3, 1), 1.0, 0.0, 3),
+    (256, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 7, 1, 3, 2, 1), 0.7, 0.3, 3),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8, 3, 2), 1.0, 0.0, 3),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 8, 4, 1), 0.9, 0.1, 3),
+    (512, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 8, 4, 1, 1, 1), 1.0, 0.0, 3),
+    (512, wl.scheme_code(wl.DEV_DTR, wl.BLK_DTR, 8, 3, 2), 0.6, 0.4, 2),
 ]
 
 
@@ -357,6 +373,8 @@ def test_batch_members_equal_their_single_runs_and_the_oracle():
              (128, wl.scheme_code(wl.DEV_DTR, wl.BLK_DT, 5), 0.7, 0.3, 3, 260),     # more members than one launch holds (256)
              (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DB, 6), 1.0, 0.0, 4, 3),
              (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 2, 2), 1.0, 0.0, 3, 4),
+             (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 6, 3, 1), 0.9, 0.1, 3, 5),
+             (128, wl.scheme_code(wl.DEV_DB, wl.BLK_DT, 6, 1, 3), 1.0, 0.0, 3, 3),
              (256, wl.scheme_code(wl.DEV_DTR, wl.BLK_DB, 7), 1.0, 0.0, 2, 3)]
     for L, code, p, q, n, members in cases:
         seeds = [500 + 7 * i for i in range(members)]
