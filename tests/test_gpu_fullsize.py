@@ -233,10 +233,13 @@ def test_whole_lattice_equals_the_oracle_at_full_size(name, kernel):
     sim.close()
 
 
-def test_config3_whole_run_equals_the_oracle():
-    """BASELINE config 3 in full: L = 4096, p = 0.9, q = 0.1, seed 7, DTrDB D = 128 (delayed borders), 5000 MCS: the
-    lattice hash every 500 MCS and (S1, S2, h00, net) after EVERY MCS (W^2(t) and the mean height per MCS)."""
-    cps, windows = read_full("c3_D128")
+@pytest.mark.parametrize("name", ["c3_D128", "c3_D64"])
+def test_config3_whole_run_equals_the_oracle(name):
+    """BASELINE config 3 in full: L = 4096, p = 0.9, q = 0.1, seed 7, DTrDB (delayed borders), 5000 MCS: the lattice hash
+    every 500 MCS and (S1, S2, h00, net) after EVERY MCS (W^2(t) and the mean height per MCS).  D = 128 is the config's own
+    shape (four warps per domain: three phases every step); D = 64 is the shape whose domains sit in one warp, where the
+    kernel decides per collective step between one pass and three phases."""
+    cps, windows = read_full(name)
     assert [c["t"] for c in cps] == list(range(500, 5001, 500)) and len(windows) == len(cps)
     c0 = cps[0]
     sim = binding.Sim(c0["L"], c0["seed"])
